@@ -1,0 +1,125 @@
+/*
+ * lbwp.h -- C ABI of the B200 (sm_100a) "lattice Boltzmann without populations" library.
+ *
+ * Method: arxiv 2301.01622 ("Lightweight Lattice Boltzmann").  Citations are
+ * PAPER.md:<line> (+ equation); "Cn" are the readings listed in DESIGN.md.
+ *
+ * One context = one periodic box on one GPU.  The state of the scheme is the set
+ * of hydrodynamic moments per node, H = [rho, u_a, P_ab] (Eq. 1-3),
+ * kept in two ping-pong device buffers ("Flip-Flop").  lbwp_step()
+ * advances it by the fused Reconstruct-Collide-Stream-Project update
+ * (Eq. 8 at the neighbour, Eq. 9 pull, Eq. 1-3 at the node).
+ *
+ * External moment layout (input of lbwp_init, output of lbwp_moments): dense SoA
+ * [M][nz][ny][nx], x fastest, element type = params.dtype.
+ *   ncomp == 1, M = 10: rho, ux, uy, uz, Pxx, Pyy, Pzz, Pxy, Pxz, Pyz
+ *   ncomp == 2, M = 11: rhoA, rhoB, ux, uy, uz, Pxx, Pyy, Pzz, Pxy, Pxz, Pyz
+ * P is the full second moment sum_i f_i c_ia c_ib (Eq. 3), u is the
+ * velocity, both of the total fluid for ncomp == 2.
+ * The internal device layout (ghost layers, row padding, deviation storage) is
+ * private to the library and not visible through this interface.
+ *
+ * Every function returns LBWP_OK (0) or a negative lbwp_status; nothing throws or
+ * aborts.  lbwp_last_error() gives the text of the calling thread's last failure.
+ * There is no CPU fallback: without a CUDA device of compute capability 10.x
+ * lbwp_init fails with LBWP_EUNSUPPORTED / LBWP_ECUDA.
+ */
+#ifndef LBWP_H
+#define LBWP_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lbwp_ctx lbwp_ctx; /* opaque; owned by the library */
+
+enum lbwp_status {
+    LBWP_OK = 0,
+    LBWP_EINVAL = -1,      /* bad argument (lattice, dtype, ncomp, sizes, tau, NULL) */
+    LBWP_ENOMEM = -2,      /* device or host allocation failed */
+    LBWP_ECUDA = -3,       /* a CUDA runtime call failed; see lbwp_last_error() */
+    LBWP_EUNSUPPORTED = -4 /* device is not sm_100, or the combination is not built */
+};
+enum lbwp_dtype { LBWP_F32 = 0, LBWP_F64 = 1 };
+enum lbwp_scheme {
+    LBWP_MOMENTS = 0,    /* the paper's scheme: moments only */
+    LBWP_POPULATIONS = 1 /* comparison point: population-storing pull BGK */
+};
+enum lbwp_kernel {
+    LBWP_KERNEL_AUTO = 0,   /* fastest kernel built for the combination */
+    LBWP_KERNEL_GATHER = 1, /* one thread per node, 27/19-neighbour gather through L1/L2 */
+    LBWP_KERNEL_MARCH = 2   /* shared-memory tiles, z-marching register accumulators */
+};
+
+typedef struct lbwp_params {
+    int32_t struct_size; /* = sizeof(lbwp_params); ABI check */
+    int32_t lattice;     /* 19 | 27  (D3Q19 is the paper's; D3Q27 reading C10) */
+    int32_t dtype;       /* lbwp_dtype: precision of the stored state AND of the arithmetic */
+    int32_t ncomp;       /* 1 | 2 (2 = colour-gradient two-component; reading C6) */
+    int32_t scheme;      /* lbwp_scheme */
+    int32_t kernel;      /* lbwp_kernel; AUTO unless a test wants a specific one */
+    int32_t nx, ny, nz;  /* periodic box (reading C13), each >= 1 */
+    int32_t device;      /* CUDA device ordinal */
+    double tau;          /* relaxation time > 0.5; omega = 1/tau, nu = cs^2 (tau - 1/2) (C3) */
+    double A;            /* ncomp == 2: perturbation (surface tension) strength; else ignored */
+    double beta;         /* ncomp == 2: recolouring strength; else ignored */
+    void *stream;        /* cudaStream_t all work is enqueued on; NULL = legacy default stream */
+    void *buf[2];        /* optional caller-owned DEVICE buffers, each >= lbwp_state_bytes() bytes and
+                            256-byte aligned (e.g. a torch tensor's data_ptr); must outlive the ctx.
+                            NULL, NULL => the library allocates and frees them. */
+} lbwp_params;
+
+/* Bytes of ONE internal state buffer (ghost layers and padding included) for these
+ * params; 0 if they are invalid.  Host-only, no CUDA call. */
+size_t lbwp_state_bytes(const lbwp_params *params);
+
+/* Number of moment fields M of the external layout (10 or 11); 0 if invalid. */
+int lbwp_num_moments(const lbwp_params *params);
+
+/* Create a context and load the initial moments (external layout above; `moments`
+ * is a HOST pointer if moments_on_device == 0, else a DEVICE pointer on
+ * params->device).  For scheme == LBWP_POPULATIONS the initial populations are the
+ * Eq. 4 reconstruction of these moments.  Synchronises the stream
+ * before returning.  *out is set only on success. */
+int lbwp_init(const lbwp_params *params, const void *moments, int moments_on_device, lbwp_ctx **out);
+
+/* Enqueue n >= 0 time steps on the context's stream; asynchronous (no sync).
+ * n == 0 is a no-op.  Launch errors are reported; execution errors surface at the
+ * next synchronising call. */
+int lbwp_step(lbwp_ctx *ctx, int64_t n);
+
+/* Write the current moments, external layout, M*nz*ny*nx elements of params.dtype,
+ * to `dst` (HOST pointer if dst_on_device == 0, else DEVICE pointer).  Synchronises
+ * the stream.  Does not change the state. */
+int lbwp_moments(lbwp_ctx *ctx, void *dst, int dst_on_device);
+
+/* Replace the state by new moments (same conventions as lbwp_init); step counter -> 0. */
+int lbwp_set_moments(lbwp_ctx *ctx, const void *moments, int moments_on_device);
+
+/* Time steps taken since init / set_moments. */
+int64_t lbwp_steps_done(const lbwp_ctx *ctx);
+
+/* Number of kernel launches lbwp_step enqueues per time step for this context
+ * (1 for the fused single-component kernels). */
+int lbwp_launches_per_step(const lbwp_ctx *ctx);
+
+/* Name of the step kernel variant in use ("march27_f32", "gather19_f64_c2", ...);
+ * static storage, never freed by the caller. */
+const char *lbwp_kernel_name(const lbwp_ctx *ctx);
+
+/* Synchronise the context's stream. */
+int lbwp_sync(lbwp_ctx *ctx);
+
+/* Free the context and every buffer the library allocated (never the caller's buf[]). */
+int lbwp_destroy(lbwp_ctx *ctx);
+
+/* Text of the calling thread's last error ("" if none); thread-local static storage. */
+const char *lbwp_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LBWP_H */

@@ -193,7 +193,7 @@ static void step_1c(const lattice_t *L, int nx, int ny, int nz, double omega, co
 /* Two-component colour-gradient step (reading C6/C7/C8,    */
 /* 105).  State: rhoA, rhoB, u, P (u, P of the total fluid).                 */
 /*  0. phi = (rhoA-rhoB)/(rhoA+rhoB);                         */
-/*     G(y) = (1/cs^2) sum_i w_i c_i phi(y+c_i); n = G/|G| (0 if |G|^2<=1e-30)*/
+/*     G(y) = (1/cs^2) sum_i w_i c_i phi(y+c_i); n = G/|G| (0 if |G|^2<=1e-10)*/
 /*  1. at y = x-c_i: h' by Eq. 8 with rho = rhoA+rhoB;                       */
 /*     perturbation  h'' = h' + (A/2)|G| [ w_i (c_i.n)^2 - B_i ],            */
 /*        B_i = w_i (i != rest), B_0 = w_0 - 2/3;                            */
@@ -231,7 +231,7 @@ static void colour_ops(const lattice_t *L, int i, double hp, double rhoA, double
     const int *c = L->c[i];
     double g2 = G[0] * G[0] + G[1] * G[1] + G[2] * G[2];
     double gn = 0.0, nvec[3] = {0, 0, 0};
-    if (g2 > 1e-30) { /* C8 */
+    if (g2 > 1e-10) { /* C8: |G| <= 1e-5 is below the fp32 noise of phi; n := 0 */
         gn = sqrt(g2);
         for (int a = 0; a < 3; ++a) nvec[a] = G[a] / gn;
     }

@@ -1,0 +1,305 @@
+// lbwp_api.cu -- the C ABI of include/lbwp.h over the sm_100a kernels.
+// Host logic only: argument checks, buffer ownership, ping-pong bookkeeping
+// ("Flip-Flop") and kernel selection.  No CPU fallback exists.
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/lbwp.h"
+#include "lbwp_common.cuh"
+#include "lbwp_convert.cuh"
+#include "lbwp_gather.cuh"
+#include "lbwp_march.cuh"
+#include "lbwp_pop.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CU(call)                                                                               \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess)                                                                 \
+            return fail(e_ == cudaErrorMemoryAllocation ? LBWP_ENOMEM : LBWP_ECUDA, "%s: %s", #call, \
+                        cudaGetErrorString(e_));                                               \
+    } while (0)
+
+bool params_ok(const lbwp_params* p) {
+    if (!p || p->struct_size != (int32_t)sizeof(lbwp_params)) return false;
+    if (p->lattice != 19 && p->lattice != 27) return false;
+    if (p->dtype != LBWP_F32 && p->dtype != LBWP_F64) return false;
+    if (p->ncomp != 1 && p->ncomp != 2) return false;
+    if (p->scheme != LBWP_MOMENTS && p->scheme != LBWP_POPULATIONS) return false;
+    if (p->kernel < LBWP_KERNEL_AUTO || p->kernel > LBWP_KERNEL_MARCH) return false;
+    if (p->nx < 1 || p->ny < 1 || p->nz < 1) return false;
+    if ((long long)p->nx * p->ny * p->nz > (1ll << 31)) return false;
+    if (!(p->tau > 0.5)) return false;  // also rejects NaN
+    if ((p->buf[0] == nullptr) != (p->buf[1] == nullptr)) return false;
+    return true;
+}
+
+int elem_bytes(const lbwp_params* p) { return p->dtype == LBWP_F32 ? 4 : 8; }
+int num_moments(const lbwp_params* p) { return p->ncomp == 1 ? 10 : 11; }
+int state_fields(const lbwp_params* p) {
+    return p->scheme == LBWP_MOMENTS ? num_moments(p) : p->ncomp * p->lattice;
+}
+
+}  // namespace
+
+struct lbwp_ctx {
+    lbwp_params P;
+    lbwp::Layout L;
+    int M = 0, nfields = 0, esize = 0;
+    void* buf[2] = {nullptr, nullptr};
+    bool owns = false;
+    void* grad = nullptr;     // ncomp==2: colour gradient scratch, 3 fields
+    void* staging = nullptr;  // dense external-layout device buffer for host <-> device I/O
+    int cur = 0;
+    int64_t steps = 0;
+    cudaStream_t stream = nullptr;
+    int variant = LBWP_KERNEL_GATHER;
+    int launches_per_step = 1;
+    char name[64] = "";
+    virtual ~lbwp_ctx() {}
+    virtual int step_once() = 0;
+    virtual int import_dense(const void* dev_ext) = 0;
+    virtual int export_dense(void* dev_ext) = 0;
+};
+
+namespace {
+
+dim3 node_grid(const lbwp::Layout& L, dim3 b) { return dim3((L.nx + b.x - 1) / b.x, (L.ny + b.y - 1) / b.y, L.nz); }
+
+template <typename T>
+struct Ctx final : lbwp_ctx {
+    lbwp::StepParams<T> sp(int from, int to) const {
+        lbwp::StepParams<T> s;
+        s.L = L;
+        s.src = (const T*)buf[from];
+        s.dst = (T*)buf[to];
+        s.grad = (const T*)grad;
+        s.omega = T(1.0 / P.tau);
+        s.A = T(P.A);
+        s.beta = T(P.beta);
+        return s;
+    }
+
+    template <int Q, int NC>
+    int step_moments(const lbwp::StepParams<T>& s) {
+        const dim3 b(32, 8, 1), g = node_grid(L, b);
+        if (NC == 2) lbwp::k_colour_gradient<T, Q><<<g, b, 0, stream>>>(s, (T*)grad);
+        if (NC == 1 && Q == 27 && variant == LBWP_KERNEL_MARCH) return lbwp::launch_march27<T>(s, stream);
+        lbwp::k_step_gather<T, Q, NC><<<g, b, 0, stream>>>(s);
+        return 0;
+    }
+
+    int step_once() override {
+        const lbwp::StepParams<T> s = sp(cur, cur ^ 1);
+        const dim3 b(32, 8, 1), g = node_grid(L, b);
+        if (P.scheme == LBWP_POPULATIONS) {
+            if (P.lattice == 27) lbwp::k_pop_step<T, 27><<<g, b, 0, stream>>>(s);
+            else lbwp::k_pop_step<T, 19><<<g, b, 0, stream>>>(s);
+        } else {
+            int rc = 0;
+            if (P.lattice == 27) rc = P.ncomp == 1 ? step_moments<27, 1>(s) : step_moments<27, 2>(s);
+            else rc = P.ncomp == 1 ? step_moments<19, 1>(s) : step_moments<19, 2>(s);
+            if (rc) return fail(LBWP_ECUDA, "march kernel launch: %s", cudaGetErrorString((cudaError_t)rc));
+        }
+        CU(cudaGetLastError());
+        cur ^= 1;
+        ++steps;
+        return LBWP_OK;
+    }
+
+    int import_dense(const void* ext) override {
+        const dim3 b(32, 8, 1), g = node_grid(L, b);
+        steps = 0;
+        if (P.scheme == LBWP_POPULATIONS) {
+            // seed F_{-1} in buf[1], then one collide pass gives F_0 in buf[0] (lbwp_pop.cuh)
+            if (P.lattice == 27) lbwp::k_pop_import<T, 27><<<g, b, 0, stream>>>(L, (const T*)ext, (T*)buf[1]);
+            else lbwp::k_pop_import<T, 19><<<g, b, 0, stream>>>(L, (const T*)ext, (T*)buf[1]);
+            CU(cudaGetLastError());
+            cur = 1;
+            int rc = step_once();
+            steps = 0;
+            return rc;
+        }
+        cur = 0;
+        if (P.ncomp == 1) lbwp::k_import_moments<T, 1><<<g, b, 0, stream>>>(L, (const T*)ext, (T*)buf[0]);
+        else lbwp::k_import_moments<T, 2><<<g, b, 0, stream>>>(L, (const T*)ext, (T*)buf[0]);
+        CU(cudaGetLastError());
+        return LBWP_OK;
+    }
+
+    int export_dense(void* ext) override {
+        const dim3 b(32, 8, 1), g = node_grid(L, b);
+        if (P.scheme == LBWP_POPULATIONS) {
+            if (P.lattice == 27) lbwp::k_pop_export<T, 27><<<g, b, 0, stream>>>(L, (const T*)buf[cur ^ 1], (T*)ext);
+            else lbwp::k_pop_export<T, 19><<<g, b, 0, stream>>>(L, (const T*)buf[cur ^ 1], (T*)ext);
+        } else if (P.ncomp == 1) {
+            lbwp::k_export_moments<T, 1><<<g, b, 0, stream>>>(L, (const T*)buf[cur], (T*)ext);
+        } else {
+            lbwp::k_export_moments<T, 2><<<g, b, 0, stream>>>(L, (const T*)buf[cur], (T*)ext);
+        }
+        CU(cudaGetLastError());
+        return LBWP_OK;
+    }
+};
+
+size_t dense_bytes(const lbwp_ctx* c) { return (size_t)c->M * c->L.nx * c->L.ny * c->L.nz * c->esize; }
+
+int load_moments(lbwp_ctx* c, const void* moments, int on_device) {
+    if (!moments) return fail(LBWP_EINVAL, "moments is NULL");
+    CU(cudaSetDevice(c->P.device));
+    const void* dev = moments;
+    if (!on_device) {
+        if (!c->staging) CU(cudaMalloc(&c->staging, dense_bytes(c)));
+        CU(cudaMemcpyAsync(c->staging, moments, dense_bytes(c), cudaMemcpyHostToDevice, c->stream));
+        dev = c->staging;
+    }
+    int rc = c->import_dense(dev);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(c->stream));
+    return LBWP_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t lbwp_state_bytes(const lbwp_params* p) {
+    if (!params_ok(p)) return 0;
+    const lbwp::Layout L = lbwp::make_layout(p->nx, p->ny, p->nz, elem_bytes(p));
+    return (size_t)state_fields(p) * (size_t)L.field * (size_t)elem_bytes(p);
+}
+
+int lbwp_num_moments(const lbwp_params* p) { return params_ok(p) ? num_moments(p) : 0; }
+
+int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, lbwp_ctx** out) {
+    if (!out) return fail(LBWP_EINVAL, "out is NULL");
+    if (!params_ok(p)) return fail(LBWP_EINVAL, "invalid lbwp_params (lattice 19|27, dtype, ncomp 1|2, sizes >= 1, tau > 0.5, struct_size)");
+    if (!moments) return fail(LBWP_EINVAL, "moments is NULL");
+    if (p->scheme == LBWP_POPULATIONS && p->ncomp != 1)
+        return fail(LBWP_EUNSUPPORTED, "population-storing comparison kernel is built for ncomp == 1 only");
+    if (p->kernel == LBWP_KERNEL_MARCH && !(p->scheme == LBWP_MOMENTS && p->ncomp == 1 && p->lattice == 27))
+        return fail(LBWP_EUNSUPPORTED, "LBWP_KERNEL_MARCH is built for D3Q27 single-component moments only");
+    int ndev = 0;
+    CU(cudaGetDeviceCount(&ndev));
+    if (p->device < 0 || p->device >= ndev) return fail(LBWP_EINVAL, "device %d out of range (%d devices)", p->device, ndev);
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, p->device));
+    if (prop.major != 10)
+        return fail(LBWP_EUNSUPPORTED, "device %d is sm_%d%d; this library is built for sm_100a only", p->device, prop.major, prop.minor);
+    CU(cudaSetDevice(p->device));
+
+    lbwp_ctx* c = p->dtype == LBWP_F32 ? (lbwp_ctx*)new (std::nothrow) Ctx<float>() : (lbwp_ctx*)new (std::nothrow) Ctx<double>();
+    if (!c) return fail(LBWP_ENOMEM, "host allocation failed");
+    c->P = *p;
+    c->esize = elem_bytes(p);
+    c->L = lbwp::make_layout(p->nx, p->ny, p->nz, c->esize);
+    c->M = num_moments(p);
+    c->nfields = state_fields(p);
+    c->stream = (cudaStream_t)p->stream;
+    const size_t bytes = lbwp_state_bytes(p);
+    int rc = LBWP_OK;
+    auto bail = [&](int code) { lbwp_destroy(c); return code; };
+    if (p->buf[0]) {
+        if (((uintptr_t)p->buf[0] | (uintptr_t)p->buf[1]) & 255) return bail(fail(LBWP_EINVAL, "buf[] must be 256-byte aligned"));
+        c->buf[0] = p->buf[0];
+        c->buf[1] = p->buf[1];
+    } else {
+        c->owns = true;
+        for (int k = 0; k < 2; ++k) {
+            cudaError_t e = cudaMalloc(&c->buf[k], bytes);
+            if (e != cudaSuccess) return bail(fail(LBWP_ENOMEM, "cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e)));
+        }
+    }
+    if (p->scheme == LBWP_MOMENTS && p->ncomp == 2) {
+        cudaError_t e = cudaMalloc(&c->grad, (size_t)3 * c->L.field * c->esize);
+        if (e != cudaSuccess) return bail(fail(LBWP_ENOMEM, "cudaMalloc(grad): %s", cudaGetErrorString(e)));
+        c->launches_per_step = 2;
+    }
+    // ghost cells and padding start defined (padding is never read by a node update)
+    for (int k = 0; k < 2; ++k) {
+        cudaError_t e = cudaMemsetAsync(c->buf[k], 0, bytes, c->stream);
+        if (e != cudaSuccess) return bail(fail(LBWP_ECUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e)));
+    }
+    const bool march_ok = p->scheme == LBWP_MOMENTS && p->ncomp == 1 && p->lattice == 27;
+    c->variant = (p->kernel == LBWP_KERNEL_AUTO) ? (march_ok ? LBWP_KERNEL_MARCH : LBWP_KERNEL_GATHER) : p->kernel;
+    snprintf(c->name, sizeof(c->name), "%s%d_%s%s",
+             p->scheme == LBWP_POPULATIONS ? "pop_pull" : (c->variant == LBWP_KERNEL_MARCH ? "march" : "gather"),
+             p->lattice, p->dtype == LBWP_F32 ? "f32" : "f64", p->ncomp == 2 ? "_c2" : "");
+    rc = load_moments(c, moments, moments_on_device);
+    if (rc) return bail(rc);
+    *out = c;
+    return LBWP_OK;
+}
+
+int lbwp_step(lbwp_ctx* c, int64_t n) {
+    if (!c || n < 0) return fail(LBWP_EINVAL, "lbwp_step: ctx NULL or n < 0");
+    if (n == 0) return LBWP_OK;
+    CU(cudaSetDevice(c->P.device));
+    for (int64_t t = 0; t < n; ++t) {
+        int rc = c->step_once();
+        if (rc) return rc;
+    }
+    return LBWP_OK;
+}
+
+int lbwp_moments(lbwp_ctx* c, void* dst, int dst_on_device) {
+    if (!c || !dst) return fail(LBWP_EINVAL, "lbwp_moments: NULL argument");
+    CU(cudaSetDevice(c->P.device));
+    void* dev = dst;
+    if (!dst_on_device) {
+        if (!c->staging) CU(cudaMalloc(&c->staging, dense_bytes(c)));
+        dev = c->staging;
+    }
+    int rc = c->export_dense(dev);
+    if (rc) return rc;
+    if (!dst_on_device) CU(cudaMemcpyAsync(dst, dev, dense_bytes(c), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return LBWP_OK;
+}
+
+int lbwp_set_moments(lbwp_ctx* c, const void* moments, int on_device) {
+    if (!c) return fail(LBWP_EINVAL, "ctx is NULL");
+    return load_moments(c, moments, on_device);
+}
+
+int64_t lbwp_steps_done(const lbwp_ctx* c) { return c ? c->steps : -1; }
+int lbwp_launches_per_step(const lbwp_ctx* c) { return c ? c->launches_per_step : 0; }
+const char* lbwp_kernel_name(const lbwp_ctx* c) { return c ? c->name : ""; }
+
+int lbwp_sync(lbwp_ctx* c) {
+    if (!c) return fail(LBWP_EINVAL, "ctx is NULL");
+    CU(cudaStreamSynchronize(c->stream));
+    return LBWP_OK;
+}
+
+int lbwp_destroy(lbwp_ctx* c) {
+    if (!c) return LBWP_OK;
+    cudaSetDevice(c->P.device);
+    cudaStreamSynchronize(c->stream);
+    if (c->owns)
+        for (int k = 0; k < 2; ++k)
+            if (c->buf[k]) cudaFree(c->buf[k]);
+    if (c->grad) cudaFree(c->grad);
+    if (c->staging) cudaFree(c->staging);
+    delete c;
+    return LBWP_OK;
+}
+
+const char* lbwp_last_error(void) { return g_err; }
+
+}  // extern "C"

@@ -39,14 +39,19 @@ def pack2(rho_a, rho_b, u):
     return np.stack([rho_a, rho_b, *u, *_pi_eq(rho_a + rho_b, u)]).astype(np.float64)
 
 
-def taylor_green(n, u0=0.01, shape=None):
-    """Config 1 / sweep: 2D-in-3D Taylor-Green vortex in x-y, rho=1, k=2*pi/nx."""
+def taylor_green(n, u0=0.01, shape=None, dtype=np.float64):
+    """Config 1 / sweep: 2D-in-3D Taylor-Green vortex in x-y, rho=1, k=2*pi/nx.  The field does not
+    depend on z, so one fp64 x-y plane is computed and broadcast (rounded to ``dtype`` on write:
+    the same values as rounding the fp64 3-D field, without its 80 B/node of host memory)."""
     nx, ny, nz = shape if shape is not None else (n, n, n)
-    x, y, _ = _grid(nx, ny, nz)
+    x, y, _ = _grid(nx, ny, 1)
     kx, ky = 2.0 * np.pi / nx, 2.0 * np.pi / ny
     ux = u0 * np.sin(kx * x) * np.cos(ky * y)
     uy = -u0 * np.cos(kx * x) * np.sin(ky * y) * (kx / ky)
-    return pack1(np.ones_like(x), (ux, uy, np.zeros_like(x)))
+    plane = pack1(np.ones_like(x), (ux, uy, np.zeros_like(x)))  # [10, 1, ny, nx]
+    out = np.empty((10, nz, ny, nx), dtype=dtype)
+    out[:] = plane
+    return out
 
 
 def _ball_wavevectors(rng, count, kmax=4):
@@ -136,7 +141,8 @@ def sweep_case(n, lattice=27, ncomp=1, dtype="f32"):
     """Config 5 instance: 1-comp = config-1 field with k=2*pi/n, tau=0.8; 2-comp = the same
     velocity field plus config-3 geometry scaled by n/128, zero approach speed, tau=1."""
     if ncomp == 1:
-        return dict(name=f"sweep_q{lattice}_c1_{dtype}_{n}", moments=taylor_green(n),
+        return dict(name=f"sweep_q{lattice}_c1_{dtype}_{n}",
+                    moments=taylor_green(n, dtype=np.float32 if dtype == "f32" else np.float64),
                     lattice=lattice, ncomp=1, tau=0.8, A=0.0, beta=0.0, steps=200, dtype=dtype)
     tg = taylor_green(n)
     m = droplets(n, [(5 * n / 16, n / 2, n / 2), (11 * n / 16, n / 2, n / 2)], 5 * n / 32,

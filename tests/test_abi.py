@@ -1,0 +1,88 @@
+"""The C-ABI library builds for sm_100a, loads, and exports every symbol include/lbwp.h declares
+(CPU only: no compute call is made)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+from paper_2301_01622_b200 import build as lbuild
+from paper_2301_01622_b200 import lbwp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    lbuild.build()
+    return lbwp.load()
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "lbwp.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(lbwp_[a-z_]+)\s*\(", text)))
+
+
+def test_header_symbols_exported(lib):
+    syms = declared_symbols()
+    assert set(syms) == set(lbwp.EXPORTS)
+    for s in syms:
+        assert getattr(lib, s) is not None
+
+
+def test_struct_matches_header(lib):
+    # field order/size of the ctypes mirror: the library itself rejects a wrong struct_size
+    p = lbwp.make_params(lattice=27, dtype="f32", ncomp=1, shape=(4, 5, 6), tau=0.8)
+    assert lib.lbwp_num_moments(ctypes.byref(p)) == 10
+    p.struct_size -= 4
+    assert lib.lbwp_num_moments(ctypes.byref(p)) == 0
+
+
+def test_state_bytes_host_only(lib):
+    p = lbwp.make_params(lattice=27, dtype="f32", ncomp=1, shape=(256, 256, 256), tau=0.8)
+    b = lbwp.state_bytes(p)
+    ideal = 10 * 4 * 256 ** 3
+    assert ideal < b < 1.12 * ideal          # one ghost layer + 32-byte row padding
+    p2 = lbwp.make_params(lattice=27, dtype="f64", ncomp=2, shape=(256, 256, 256), tau=1.0)
+    assert lbwp.state_bytes(p2) > 11 * 8 * 256 ** 3
+    pp = lbwp.make_params(lattice=19, dtype="f32", ncomp=1, shape=(64, 64, 64), tau=0.8, scheme="populations")
+    assert lbwp.state_bytes(pp) > 19 * 4 * 64 ** 3
+
+
+@pytest.mark.parametrize("bad", [dict(lattice=15), dict(tau=0.5), dict(tau=float("nan")), dict(ncomp=3),
+                                 dict(shape=(0, 4, 4))])
+def test_invalid_params_rejected(lib, bad):
+    kw = dict(lattice=27, dtype="f32", ncomp=1, shape=(4, 4, 4), tau=0.8)
+    kw.update(bad)
+    p = lbwp.make_params(**kw)
+    assert lbwp.state_bytes(p) == 0
+    ctx = ctypes.c_void_p()
+    buf = (ctypes.c_float * 640)()
+    rc = lib.lbwp_init(ctypes.byref(p), buf, 0, ctypes.byref(ctx))
+    assert rc == -1 and not ctx.value
+    assert b"invalid" in lib.lbwp_last_error()
+
+
+def test_no_cpu_fallback(lib):
+    """Without a GPU lbwp_init must fail loudly, not compute on the host."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    p = lbwp.make_params(lattice=27, dtype="f32", ncomp=1, shape=(4, 4, 4), tau=0.8)
+    ctx = ctypes.c_void_p()
+    buf = (ctypes.c_float * 640)()
+    rc = lib.lbwp_init(ctypes.byref(p), buf, 0, ctypes.byref(ctx))
+    assert rc in (-3, -4) and not ctx.value
+    with pytest.raises(lbwp.LbwpError):
+        import numpy as np
+        lbwp.Lbwp(np.zeros((10, 4, 4, 4), np.float32), tau=0.8)
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2301_01622_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "lbwp_oracle" not in src, f
