@@ -14,6 +14,7 @@
 #include "lbwp_gather.cuh"
 #include "lbwp_march.cuh"
 #include "lbwp_pop.cuh"
+#include "lbwp_tma_host.cuh"
 
 namespace {
 
@@ -41,7 +42,7 @@ bool params_ok(const lbwp_params* p) {
     if (p->dtype != LBWP_F32 && p->dtype != LBWP_F64) return false;
     if (p->ncomp != 1 && p->ncomp != 2) return false;
     if (p->scheme != LBWP_MOMENTS && p->scheme != LBWP_POPULATIONS) return false;
-    if (p->kernel < LBWP_KERNEL_AUTO || p->kernel > LBWP_KERNEL_MARCH) return false;
+    if (p->kernel < LBWP_KERNEL_AUTO || p->kernel > LBWP_KERNEL_TMA) return false;
     if (p->nx < 1 || p->ny < 1 || p->nz < 1) return false;
     if ((long long)p->nx * p->ny * p->nz > (1ll << 31)) return false;
     if (!(p->tau > 0.5)) return false;  // also rejects NaN
@@ -53,6 +54,24 @@ int elem_bytes(const lbwp_params* p) { return p->dtype == LBWP_F32 ? 4 : 8; }
 int num_moments(const lbwp_params* p) { return p->ncomp == 1 ? 10 : 11; }
 int state_fields(const lbwp_params* p) {
     return p->scheme == LBWP_MOMENTS ? num_moments(p) : p->ncomp * p->lattice;
+}
+
+
+bool tma_eligible(const lbwp_params* p) {
+    if (!(p->scheme == LBWP_MOMENTS && p->ncomp == 1 && p->lattice == 27)) return false;
+    return p->dtype == LBWP_F32 ? lbwp::TmaPlan<float>::eligible(p->nx, p->ny, p->nz)
+                                : lbwp::TmaPlan<double>::eligible(p->nx, p->ny, p->nz);
+}
+
+// kernel variant a context with these params runs (LBWP_KERNEL_AUTO resolved); 0 if not built
+int choose_variant(const lbwp_params* p) {
+    const bool march_ok = p->scheme == LBWP_MOMENTS && p->ncomp == 1 && p->lattice == 27;
+    switch (p->kernel) {
+        case LBWP_KERNEL_AUTO: return tma_eligible(p) ? LBWP_KERNEL_TMA : march_ok ? LBWP_KERNEL_MARCH : LBWP_KERNEL_GATHER;
+        case LBWP_KERNEL_TMA: return tma_eligible(p) ? LBWP_KERNEL_TMA : 0;
+        case LBWP_KERNEL_MARCH: return march_ok ? LBWP_KERNEL_MARCH : 0;
+        default: return LBWP_KERNEL_GATHER;
+    }
 }
 
 }  // namespace
@@ -157,6 +176,48 @@ struct Ctx final : lbwp_ctx {
     }
 };
 
+// Context of the TMA variant: buf[] hold the S-form in XLayout (lbwp_tma.cuh).  buf[cur] = S-form of
+// the moments at the current time t; buf[cur^1] = S-form of time t-1 (t >= 1), or the plain moments
+// themselves (t = 0), which is what lbwp_moments needs in either case.
+template <typename T>
+struct TmaCtx final : lbwp_ctx {
+    lbwp::TmaPlan<T> plan;
+    lbwp::XLayout X;
+
+    int prepare() {
+        int rc = plan.setup(X, buf);
+        if (rc) return fail(rc < 0 ? LBWP_EUNSUPPORTED : LBWP_ECUDA, "TMA plan setup failed (%d): %s", rc,
+                            rc < 0 ? "cuTensorMapEncodeTiled not available" : "tensor map / attribute error");
+        return LBWP_OK;
+    }
+    int step_once() override {
+        int rc = plan.template launch<lbwp::EPI_SFORM>(cur, (T*)buf[cur ^ 1], T(1.0 / P.tau), stream);
+        if (rc) return fail(LBWP_ECUDA, "tma step launch: %s", cudaGetErrorString((cudaError_t)rc));
+        cur ^= 1;
+        ++steps;
+        return LBWP_OK;
+    }
+    int import_dense(const void* ext) override {
+        const dim3 b(32, 8, 1), g((X.nx + 31) / 32, (X.ny + 7) / 8, X.nz);
+        steps = 0;
+        cur = 0;
+        lbwp::k_tma_import<T><<<g, b, 0, stream>>>(X, (const T*)ext, (T*)buf[0], (T*)buf[1], T(1.0 / P.tau));
+        CU(cudaGetLastError());
+        return LBWP_OK;
+    }
+    int export_dense(void* ext) override {
+        if (steps == 0) {
+            const dim3 b(32, 8, 1), g((X.nx + 31) / 32, (X.ny + 7) / 8, X.nz);
+            lbwp::k_tma_export_raw<T><<<g, b, 0, stream>>>(X, (const T*)buf[cur ^ 1], (T*)ext);
+            CU(cudaGetLastError());
+            return LBWP_OK;
+        }
+        int rc = plan.template launch<lbwp::EPI_MOMENTS>(cur ^ 1, (T*)ext, T(1.0 / P.tau), stream);
+        if (rc) return fail(LBWP_ECUDA, "tma export launch: %s", cudaGetErrorString((cudaError_t)rc));
+        return LBWP_OK;
+    }
+};
+
 size_t dense_bytes(const lbwp_ctx* c) { return (size_t)c->M * c->L.nx * c->L.ny * c->L.nz * c->esize; }
 
 int load_moments(lbwp_ctx* c, const void* moments, int on_device) {
@@ -180,6 +241,12 @@ extern "C" {
 
 size_t lbwp_state_bytes(const lbwp_params* p) {
     if (!params_ok(p)) return 0;
+    const int variant = choose_variant(p);
+    if (variant == 0) return 0;
+    if (variant == LBWP_KERNEL_TMA) {
+        const lbwp::XLayout X = lbwp::make_xlayout(p->nx, p->ny, p->nz, elem_bytes(p));
+        return (size_t)10 * (size_t)X.field * (size_t)elem_bytes(p);
+    }
     const lbwp::Layout L = lbwp::make_layout(p->nx, p->ny, p->nz, elem_bytes(p));
     return (size_t)state_fields(p) * (size_t)L.field * (size_t)elem_bytes(p);
 }
@@ -192,8 +259,10 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
     if (!moments) return fail(LBWP_EINVAL, "moments is NULL");
     if (p->scheme == LBWP_POPULATIONS && p->ncomp != 1)
         return fail(LBWP_EUNSUPPORTED, "population-storing comparison kernel is built for ncomp == 1 only");
-    if (p->kernel == LBWP_KERNEL_MARCH && !(p->scheme == LBWP_MOMENTS && p->ncomp == 1 && p->lattice == 27))
-        return fail(LBWP_EUNSUPPORTED, "LBWP_KERNEL_MARCH is built for D3Q27 single-component moments only");
+    const int variant = choose_variant(p);
+    if (variant == 0)
+        return fail(LBWP_EUNSUPPORTED, "kernel %d is not built for this combination (MARCH/TMA: D3Q27 single-component "
+                    "moments; TMA also needs nx %% 64 (fp32) or 32 (fp64) == 0 and ny %% 8 == 0)", p->kernel);
     int ndev = 0;
     CU(cudaGetDeviceCount(&ndev));
     if (p->device < 0 || p->device >= ndev) return fail(LBWP_EINVAL, "device %d out of range (%d devices)", p->device, ndev);
@@ -203,7 +272,14 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
         return fail(LBWP_EUNSUPPORTED, "device %d is sm_%d%d; this library is built for sm_100a only", p->device, prop.major, prop.minor);
     CU(cudaSetDevice(p->device));
 
-    lbwp_ctx* c = p->dtype == LBWP_F32 ? (lbwp_ctx*)new (std::nothrow) Ctx<float>() : (lbwp_ctx*)new (std::nothrow) Ctx<double>();
+    lbwp_ctx* c = nullptr;
+    if (variant == LBWP_KERNEL_TMA) {
+        const lbwp::XLayout X = lbwp::make_xlayout(p->nx, p->ny, p->nz, elem_bytes(p));
+        if (p->dtype == LBWP_F32) { auto* t = new (std::nothrow) TmaCtx<float>(); if (t) t->X = X; c = t; }
+        else { auto* t = new (std::nothrow) TmaCtx<double>(); if (t) t->X = X; c = t; }
+    } else {
+        c = p->dtype == LBWP_F32 ? (lbwp_ctx*)new (std::nothrow) Ctx<float>() : (lbwp_ctx*)new (std::nothrow) Ctx<double>();
+    }
     if (!c) return fail(LBWP_ENOMEM, "host allocation failed");
     c->P = *p;
     c->esize = elem_bytes(p);
@@ -235,10 +311,13 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
         cudaError_t e = cudaMemsetAsync(c->buf[k], 0, bytes, c->stream);
         if (e != cudaSuccess) return bail(fail(LBWP_ECUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e)));
     }
-    const bool march_ok = p->scheme == LBWP_MOMENTS && p->ncomp == 1 && p->lattice == 27;
-    c->variant = (p->kernel == LBWP_KERNEL_AUTO) ? (march_ok ? LBWP_KERNEL_MARCH : LBWP_KERNEL_GATHER) : p->kernel;
+    c->variant = variant;
+    if (variant == LBWP_KERNEL_TMA) {
+        rc = p->dtype == LBWP_F32 ? static_cast<TmaCtx<float>*>(c)->prepare() : static_cast<TmaCtx<double>*>(c)->prepare();
+        if (rc) return bail(rc);
+    }
     snprintf(c->name, sizeof(c->name), "%s%d_%s%s",
-             p->scheme == LBWP_POPULATIONS ? "pop_pull" : (c->variant == LBWP_KERNEL_MARCH ? "march" : "gather"),
+             p->scheme == LBWP_POPULATIONS ? "pop_pull" : (variant == LBWP_KERNEL_TMA ? "tma" : variant == LBWP_KERNEL_MARCH ? "march" : "gather"),
              p->lattice, p->dtype == LBWP_F32 ? "f32" : "f64", p->ncomp == 2 ? "_c2" : "");
     rc = load_moments(c, moments, moments_on_device);
     if (rc) return bail(rc);

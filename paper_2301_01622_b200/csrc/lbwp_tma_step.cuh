@@ -1,0 +1,145 @@
+// lbwp_tma_step.cuh -- kernel body of the TMA-fed D3Q27 stencil step (see lbwp_tma.cuh).
+#pragma once
+#include "lbwp_tma.cuh"
+
+namespace lbwp {
+
+enum { EPI_SFORM = 0, EPI_MOMENTS = 1 };
+
+template <typename T>
+struct TmaStepParams {
+    XLayout L;
+    T* __restrict__ dst;   // EPI_SFORM: XLayout fields; EPI_MOMENTS: dense external [10][nz][ny][nx]
+    T omega;               // 1/tau (reading C3)
+    int lz;                // z planes per chunk
+};
+
+// Compile-time geometry of one instance.
+template <typename T, int NPT_, int TX_, int TY_, int NS_>
+struct TmaCfg {
+    static constexpr int NPT = NPT_, TX = TX_, TY = TY_, NS = NS_, M = 10;
+    static constexpr int OX = 16 / (int)sizeof(T);            // halo column sits at OX-1 and OX+TX
+    static constexpr int BW = TX + 2 * OX;                    // box width: 16-byte multiple
+    static constexpr int ROW = M * BW;                        // elements per tile row [field][BW]
+    static constexpr int ROWS_T = TY / NPT;                   // thread rows
+    static constexpr int NT = TX * ROWS_T;
+    static constexpr int NW = NT / 32;
+    static constexpr int OFF_YM = TY * ROW;                   // halo row y0-1 (elements)
+    static constexpr int OFF_YP = ((((TY + 1) * ROW * (int)sizeof(T)) + 127) / 128) * 128 / (int)sizeof(T);
+    static constexpr int STAGE = (((OFF_YP + ROW) * (int)sizeof(T) + 127) / 128) * 128 / (int)sizeof(T);
+    static constexpr uint32_t STAGE_TX_BYTES = (uint32_t)((TY + 2) * ROW * sizeof(T));
+    static constexpr size_t SMEM = (size_t)NS * STAGE * sizeof(T) + 2 * NS * 8 + 128;
+    static_assert((TY * ROW * sizeof(T)) % 128 == 0, "halo row must start 128-byte aligned");
+    static_assert(NT % 32 == 0 && TY % NPT == 0, "tile/threads");
+};
+
+// x-pass of the separable (1,4,1) kernels over three brackets at cx = -1, 0, +1
+template <typename V>
+struct XRow { V r0, r1, r2; };
+template <typename V>
+__device__ __forceinline__ XRow<V> xpass(const V& m, const V& c, const V& p, const V& four) {
+    XRow<V> r;
+    r.r2 = p + m;
+    r.r1 = p - m;
+    r.r0 = vfma(four, c, r.r2);
+    return r;
+}
+
+// In-plane moments m_pq = sum k(cx) k(cy) cx^p cy^q B(cx,cy) of one bracket family
+template <typename V>
+struct Mom6 { V m00, m10, m01, m20, m02, m11; };
+template <typename V>
+__device__ __forceinline__ Mom6<V> ypass(const XRow<V>& lo, const XRow<V>& mid, const XRow<V>& hi, const V& four) {
+    Mom6<V> m;
+    m.m02 = hi.r0 + lo.r0;
+    m.m01 = hi.r0 - lo.r0;
+    m.m00 = vfma(four, mid.r0, m.m02);
+    m.m10 = vfma(four, mid.r1, hi.r1 + lo.r1);
+    m.m11 = hi.r1 - lo.r1;
+    m.m20 = vfma(four, mid.r2, hi.r2 + lo.r2);
+    return m;
+}
+
+template <typename T, typename C>
+struct TmaStep {
+    using V = Vec<T, C::NPT>;
+    static constexpr int BW = C::BW;
+
+    // value of field f at (cx, row slot j) relative to the thread's nodes: source node x - c
+    template <int F, int CX>
+    __device__ static __forceinline__ V ld(const T* __restrict__ s, const int (&r)[C::NPT][3], int j) {
+        V v;
+#pragma unroll
+        for (int n = 0; n < C::NPT; ++n) v.set(n, s[r[n][j] + F * BW - CX]);
+        return v;
+    }
+
+    // brackets of one source row (cy = CY): E, W = E + Szz, O at cx = -1, 0, +1, then the x-pass
+    template <int CY>
+    __device__ static __forceinline__ void row(const T* __restrict__ s, const int (&r)[C::NPT][3], const V& four,
+                                               XRow<V>& re, XRow<V>& rw, XRow<V>& ro) {
+        constexpr int J = 1 - CY;  // row slot of source y - cy: slot 0 = y-1, 1 = y, 2 = y+1
+        V E[3], W[3], O[3];
+#pragma unroll
+        for (int cx = -1; cx <= 1; ++cx) {
+            V e, o, z;
+            if (cx == -1) { e = ld<0, -1>(s, r, J); o = ld<3, -1>(s, r, J); z = ld<6, -1>(s, r, J);
+                            e = e + ld<4, -1>(s, r, J); e = e - ld<1, -1>(s, r, J); o = o - ld<8, -1>(s, r, J); }
+            if (cx == 0) { e = ld<0, 0>(s, r, J); o = ld<3, 0>(s, r, J); z = ld<6, 0>(s, r, J); }
+            if (cx == 1) { e = ld<0, 1>(s, r, J); o = ld<3, 1>(s, r, J); z = ld<6, 1>(s, r, J);
+                           e = e + ld<4, 1>(s, r, J); e = e + ld<1, 1>(s, r, J); o = o + ld<8, 1>(s, r, J); }
+            if (CY != 0) {
+                V syy, jy, syz;
+                if (cx == -1) { syy = ld<5, -1>(s, r, J); jy = ld<2, -1>(s, r, J); syz = ld<9, -1>(s, r, J); }
+                if (cx == 0) { syy = ld<5, 0>(s, r, J); jy = ld<2, 0>(s, r, J); syz = ld<9, 0>(s, r, J); }
+                if (cx == 1) { syy = ld<5, 1>(s, r, J); jy = ld<2, 1>(s, r, J); syz = ld<9, 1>(s, r, J); }
+                e = e + syy;
+                e = CY > 0 ? e + jy : e - jy;
+                o = CY > 0 ? o + syz : o - syz;
+                if (cx != 0) {
+                    V sxy = cx == -1 ? ld<7, -1>(s, r, J) : ld<7, 1>(s, r, J);
+                    e = (cx * CY > 0) ? e + sxy : e - sxy;
+                }
+            }
+            E[cx + 1] = e;
+            W[cx + 1] = e + z;
+            O[cx + 1] = o;
+        }
+        re = xpass<V>(E[0], E[1], E[2], four);
+        rw = xpass<V>(W[0], W[1], W[2], four);
+        ro = xpass<V>(O[0], O[1], O[2], four);
+    }
+
+    // consume one S-form input plane z: last contribution to output plane z-1 (P), middle one to
+    // plane z (C), first one to plane z+1 (N, assigned).  Order: rho, jx, jy, jz, pxx, pyy, pzz, pxy, pxz, pyz
+    __device__ static __forceinline__ void consume(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[10],
+                                                   V (&Cc)[10], V (&N)[10]) {
+        const V four = V::bc(T(4));
+        XRow<V> el, ew, eo, ml, mw_, mo_, hl, hw, ho;
+        row<-1>(s, r, four, el, ew, eo);   // sources at y+1 (cy = -1)
+        row<1>(s, r, four, hl, hw, ho);    // sources at y-1 (cy = +1)
+        row<0>(s, r, four, ml, mw_, mo_);
+        const Mom6<V> me = ypass<V>(el, ml, hl, four);
+        const Mom6<V> mw = ypass<V>(ew, mw_, hw, four);
+        const Mom6<V> mo = ypass<V>(eo, mo_, ho, four);
+        // cz = 0 (k = 4)
+        Cc[0] = vfma(four, me.m00, Cc[0]);
+        Cc[1] = vfma(four, me.m10, Cc[1]);
+        Cc[2] = vfma(four, me.m01, Cc[2]);
+        Cc[4] = vfma(four, me.m20, Cc[4]);
+        Cc[5] = vfma(four, me.m02, Cc[5]);
+        Cc[7] = vfma(four, me.m11, Cc[7]);
+        // cz = +1: arrives at plane z+1
+        const V p00 = mw.m00 + mo.m00, p10 = mw.m10 + mo.m10, p01 = mw.m01 + mo.m01;
+        N[0] = p00; N[1] = p10; N[2] = p01; N[3] = p00;
+        N[4] = mw.m20 + mo.m20; N[5] = mw.m02 + mo.m02; N[6] = p00;
+        N[7] = mw.m11 + mo.m11; N[8] = p10; N[9] = p01;
+        // cz = -1: arrives at plane z-1
+        const V n00 = mw.m00 - mo.m00, n10 = mw.m10 - mo.m10, n01 = mw.m01 - mo.m01;
+        P[0] = P[0] + n00; P[1] = P[1] + n10; P[2] = P[2] + n01; P[3] = P[3] - n00;
+        P[4] = P[4] + (mw.m20 - mo.m20); P[5] = P[5] + (mw.m02 - mo.m02); P[6] = P[6] + n00;
+        P[7] = P[7] + (mw.m11 - mo.m11); P[8] = P[8] - n10; P[9] = P[9] - n01;
+    }
+};
+
+}  // namespace lbwp

@@ -102,7 +102,7 @@ def check(lbwp, oracle, cfg, steps, kernel="auto", scheme="moments", tol=None):
 
 
 # ---- config 1: D3Q27, 32^3, fp64, tau=0.8, Taylor-Green, 100 steps ------------------------
-@pytest.mark.parametrize("kernel", ["march", "gather"])
+@pytest.mark.parametrize("kernel", ["tma", "march", "gather"])
 def test_config1_taylor_green_fp64(lbwp, oracle, kernel):
     check(lbwp, oracle, wl.config1(), 100, kernel=kernel)
 
@@ -115,6 +115,37 @@ def test_config2_ragged(lbwp, oracle, dtype, lattice, kernel):
     cfg = dict(name="config2_ragged", moments=wl.noisy_solenoidal(0, shape=(45, 38, 41)), lattice=lattice,
                ncomp=1, tau=0.6, A=0.0, beta=0.0, dtype=dtype)
     check(lbwp, oracle, cfg, 60, kernel=kernel)
+
+
+# ---- the TMA kernel: tiles in x and y, ragged z chunks, thin boxes (wrap planes coincide) ------
+@pytest.mark.parametrize("dtype,shape", [("f32", (128, 24, 37)), ("f32", (64, 8, 1)), ("f32", (64, 16, 2)),
+                                         ("f32", (192, 40, 3)), ("f64", (64, 24, 21)), ("f64", (32, 8, 1)),
+                                         ("f64", (96, 16, 2))])
+@pytest.mark.parametrize("steps", [1, 2, 25])
+def test_tma_kernel_shapes(lbwp, oracle, dtype, shape, steps):
+    cfg = dict(name="tma_%s_%s" % (dtype, "x".join(map(str, shape))), moments=wl.noisy_solenoidal(0, shape=shape),
+               lattice=27, ncomp=1, tau=0.6, A=0.0, beta=0.0, dtype=dtype)
+    check(lbwp, oracle, cfg, steps, kernel="tma")
+
+
+def test_tma_tau_one_and_restart(lbwp, oracle):
+    """tau = 1 makes the stored S-form independent of Pi (pin P6): lbwp_moments must still return the
+    pre-collision Pi of the current step; set_moments restarts the step counter and the t = 0 export."""
+    shape = (64, 16, 9)
+    m0 = wl.as_dtype(wl.noisy_solenoidal(0, shape=shape), "f64")
+    m0[4:] += 1e-3 * np.random.default_rng(5).uniform(-1, 1, m0[4:].shape)   # off-equilibrium Pi
+    with lbwp.Lbwp(m0, lattice=27, dtype="f64", tau=1.0, kernel="tma") as sim:
+        assert sim.kernel_name == "tma27_f64"
+        assert np.array_equal(sim.moments_host(), m0)
+        sim.step(3)
+        got = sim.moments_host()
+        ref = oracle.run(m0, lattice=27, tau=1.0, nsteps=3)
+        assert parity_errors(got, ref, 1, "f64").max() <= 1e-12
+        sim.set_moments(got)
+        assert sim.steps_done == 0 and np.array_equal(sim.moments_host(), got)
+        sim.step(2)
+        ref5 = oracle.run(got, lattice=27, tau=1.0, nsteps=2)
+        assert parity_errors(sim.moments_host(), ref5, 1, "f64").max() <= 1e-12
 
 
 # ---- config 2 itself: 128^3, tau=0.6, fp32 and fp64.  The oracle runs at a few MLUPS, so the
