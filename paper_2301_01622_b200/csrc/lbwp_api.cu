@@ -59,8 +59,7 @@ int state_fields(const lbwp_params* p) {
 
 bool tma_eligible(const lbwp_params* p) {
     if (!(p->scheme == LBWP_MOMENTS && p->ncomp == 1 && p->lattice == 27)) return false;
-    return p->dtype == LBWP_F32 ? lbwp::TmaPlan<float>::eligible(p->nx, p->ny, p->nz)
-                                : lbwp::TmaPlan<double>::eligible(p->nx, p->ny, p->nz);
+    return p->dtype == LBWP_F32 ? lbwp::tma_eligible_f32(p->nx, p->ny) : lbwp::tma_eligible_f64(p->nx, p->ny);
 }
 
 // kernel variant a context with these params runs (LBWP_KERNEL_AUTO resolved); 0 if not built
@@ -181,17 +180,20 @@ struct Ctx final : lbwp_ctx {
 // themselves (t = 0), which is what lbwp_moments needs in either case.
 template <typename T>
 struct TmaCtx final : lbwp_ctx {
-    lbwp::TmaPlan<T> plan;
+    lbwp::TmaPlanBase* planp = nullptr;
     lbwp::XLayout X;
+    ~TmaCtx() override { delete planp; }
 
     int prepare() {
-        int rc = plan.setup(X, buf);
+        planp = lbwp::make_tma_plan<T>(X.nx, X.ny);
+        if (!planp) return fail(LBWP_ENOMEM, "no TMA plan");
+        int rc = planp->setup(X, buf);
         if (rc) return fail(rc < 0 ? LBWP_EUNSUPPORTED : LBWP_ECUDA, "TMA plan setup failed (%d): %s", rc,
                             rc < 0 ? "cuTensorMapEncodeTiled not available" : "tensor map / attribute error");
         return LBWP_OK;
     }
     int step_once() override {
-        int rc = plan.template launch<lbwp::EPI_SFORM>(cur, (T*)buf[cur ^ 1], T(1.0 / P.tau), stream);
+        int rc = planp->launch(lbwp::EPI_SFORM, cur, buf[cur ^ 1], 1.0 / P.tau, stream);
         if (rc) return fail(LBWP_ECUDA, "tma step launch: %s", cudaGetErrorString((cudaError_t)rc));
         cur ^= 1;
         ++steps;
@@ -212,7 +214,7 @@ struct TmaCtx final : lbwp_ctx {
             CU(cudaGetLastError());
             return LBWP_OK;
         }
-        int rc = plan.template launch<lbwp::EPI_MOMENTS>(cur ^ 1, (T*)ext, T(1.0 / P.tau), stream);
+        int rc = planp->launch(lbwp::EPI_MOMENTS, cur ^ 1, ext, 1.0 / P.tau, stream);
         if (rc) return fail(LBWP_ECUDA, "tma export launch: %s", cudaGetErrorString((cudaError_t)rc));
         return LBWP_OK;
     }

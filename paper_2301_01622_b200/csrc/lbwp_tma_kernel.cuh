@@ -54,8 +54,39 @@ __device__ __forceinline__ void epilogue_node(const TmaStepParams<T>& p, const T
     }
 }
 
+// Work decomposition: item = (z chunk, tile row, tile column), x fastest, so that items handled at
+// the same time by neighbouring CTAs are spatial neighbours and their halo reads meet in L2.
+struct TmaItem {
+    int x0, y0, z0, nin, ym, yp;
+};
+template <typename C>
+__device__ __forceinline__ TmaItem tma_item(const XLayout& L, int lz, int gx, int gy, int item) {
+    TmaItem t;
+    const int tx = item % gx, r = item / gx;
+    const int ty = r % gy, tz = r / gy;
+    t.x0 = tx * C::TX;
+    t.y0 = ty * C::TY;
+    t.z0 = tz * lz;
+    t.nin = min(lz, L.nz - t.z0) + 2;                       // input planes z0-1 .. z1
+    t.ym = t.y0 == 0 ? L.ny - 1 : t.y0 - 1;                 // halo rows wrap in y (reading C13)
+    t.yp = t.y0 + C::TY >= L.ny ? 0 : t.y0 + C::TY;
+    return t;
+}
+
+// CTA b handles items b, b + gridDim.x, ... (gridDim.x = number of items gives one item per CTA and
+// leaves the order to the hardware scheduler; a smaller grid makes the CTAs persistent).  Warp
+// specialisation: the last warp is the TMA producer (one elected lane), the first NW warps consume.  The
+// stage ring runs straight across item boundaries.
+// registers per thread that still let MINB CTAs of NT + 32 threads share an SM's 64 K registers
+// (warps are placed four at a time, one per scheduler, so a CTA of 17 warps is budgeted as 20)
+__host__ __device__ constexpr int tma_max_regs(int threads, int minb) {
+    const int warps = (threads / 32 + 3) / 4 * 4;
+    const int r = 65536 / (minb * warps * 32) / 8 * 8;
+    return r > 248 ? 248 : r;
+}
+
 template <typename T, typename C, int EPI, int MINB>
-__global__ void __launch_bounds__(C::NT, MINB)
+__global__ void __maxnreg__(tma_max_regs(C::NT + 32, MINB))
 k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant__ CUtensorMap map_row,
              const TmaStepParams<T> p) {
     using S = TmaStep<T, C>;
@@ -70,13 +101,10 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
 
     const XLayout& L = p.L;
     const int tid = threadIdx.x;
-    const int tx = tid % C::TX, tr = tid / C::TX;
-    const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
-    const int z0 = blockIdx.z * p.lz;
-    const int z1 = min(z0 + p.lz, L.nz);
-    const int nin = z1 - z0 + 2;                 // input planes z0-1 .. z1
-    const int ym = y0 == 0 ? L.ny - 1 : y0 - 1;   // halo rows wrap in y (reading C13)
-    const int yp = y0 + C::TY >= L.ny ? 0 : y0 + C::TY;
+    const int gx = L.nx / C::TX, gy = L.ny / C::TY;
+    const int nitems = gx * gy * ((L.nz + p.lz - 1) / p.lz);
+    int item = blockIdx.x;
+    if (item >= nitems) return;
 
     if (tid == 0) {
 #pragma unroll
@@ -85,21 +113,30 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
     }
     __syncthreads();
 
-    auto issue = [&](int i, int s) {   // input plane index i -> stage s (thread 0 only)
-        int z = z0 - 1 + i;
-        z = z < 0 ? z + L.nz : (z >= L.nz ? z - L.nz : z);
-        const uint32_t dst = base + (uint32_t)(s * C::STAGE * sizeof(T));
-        mbar_expect_tx(full(s), C::STAGE_TX_BYTES);
-        tma_load_4d(dst, &map_main, full(s), x0, 0, y0, z);
-        tma_load_4d(dst + (uint32_t)(C::OFF_YM * sizeof(T)), &map_row, full(s), x0, 0, ym, z);
-        tma_load_4d(dst + (uint32_t)(C::OFF_YP * sizeof(T)), &map_row, full(s), x0, 0, yp, z);
-    };
-    if (tid == 0) {
-#pragma unroll
-        for (int i = 0; i < C::NS - 1; ++i)
-            if (i < nin) issue(i, i);
+    if (tid >= C::NT) {
+        // ---- producer warp: fills every free stage, up to NS planes ahead of the consumers ----
+        if (tid != C::NT) return;
+        int ps = 0;
+        uint32_t pround = 0;
+        for (; item < nitems; item += gridDim.x) {
+            const TmaItem t = tma_item<C>(L, p.lz, gx, gy, item);
+            for (int i = 0; i < t.nin; ++i) {
+                if (pround > 0) mbar_wait(empty(ps), (pround - 1u) & 1u);   // previous use released
+                int z = t.z0 - 1 + i;
+                z = z < 0 ? z + L.nz : (z >= L.nz ? z - L.nz : z);          // z wraps on the load side
+                const uint32_t dst = base + (uint32_t)(ps * C::STAGE * sizeof(T));
+                mbar_expect_tx(full(ps), C::STAGE_TX_BYTES);
+                tma_load_4d(dst, &map_main, full(ps), t.x0, 0, t.y0, z);
+                tma_load_4d(dst + (uint32_t)(C::OFF_YM * sizeof(T)), &map_row, full(ps), t.x0, 0, t.ym, z);
+                tma_load_4d(dst + (uint32_t)(C::OFF_YP * sizeof(T)), &map_row, full(ps), t.x0, 0, t.yp, z);
+                if (++ps == C::NS) { ps = 0; ++pround; }
+            }
+        }
+        return;
     }
 
+    // ---- consumer warps ----
+    const int tx = tid % C::TX, tr = tid / C::TX;
     // element offsets (within a stage) of the three source rows of each owned node, at x = tx
     int r[C::NPT][3];
 #pragma unroll
@@ -116,45 +153,56 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
 #pragma unroll
     for (int f = 0; f < 10; ++f) a0[f] = a1[f] = a2[f] = V::bc(T(0));
 
-    const int x = x0 + tx;
-    int i = 0;   // input plane counter
+    TmaItem ct = tma_item<C>(L, p.lz, gx, gy, item);
+    int i = 0;            // input plane counter within the item
+    int s = 0;            // stage of the current plane
+    uint32_t par = 0;     // phase parity of this round of the ring
 
-    auto plane = [&](V(&P)[10], V(&Cc)[10], V(&N)[10], int s, uint32_t par) {
-        if (tid == 0) {
-            const int j = i + C::NS - 1;            // refill the stage freed one plane ago
-            if (j < nin) {
-                const int sj = (s + C::NS - 1) % C::NS;
-                if (j >= C::NS) mbar_wait(empty(sj), ((uint32_t)(j / C::NS) - 1u) & 1u);
-                issue(j, sj);
-            }
-        }
+    // The first two planes of an item only prime the accumulators (their "finished" planes belong to
+    // the z halo and are not stored), so nothing has to be reset at an item boundary.
+    auto plane = [&](V(&P)[10], V(&Cc)[10], V(&N)[10]) {
+        int rs[C::NPT][3];
+#pragma unroll
+        for (int n = 0; n < C::NPT; ++n)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) rs[n][j] = r[n][j] + s * C::STAGE;
         mbar_wait(full(s), par);
-        S::consume(sm + s * C::STAGE, r, P, Cc, N);
+#ifdef LBWP_TMA_PROBE_NOCOMPUTE   // tuning probe only: memory-side ceiling of this access pattern
+#pragma unroll
+        for (int f = 0; f < 10; ++f) {
+#pragma unroll
+            for (int n = 0; n < C::NPT; ++n) N[f].set(n, sm[rs[n][1] + f * C::BW] + sm[rs[n][0] + f * C::BW - 1] + sm[rs[n][2] + f * C::BW + 1]);
+            P[f] = P[f] + Cc[f];
+        }
+#else
+        S::consume(sm, rs, P, Cc, N);
+#endif
         __syncwarp();
         if ((tid & 31) == 0) mbar_arrive(empty(s));
-        const int zo = z0 + i - 2;                  // plane completed by this input plane
-        if (zo >= z0) {
+        if (i >= 2) {                               // this input plane completes output plane z0 + i - 2
 #pragma unroll
             for (int n = 0; n < C::NPT; ++n) {
                 T acc[10];
 #pragma unroll
                 for (int f = 0; f < 10; ++f) acc[f] = P[f].get(n);
-                epilogue_node<T, EPI>(p, acc, x, y0 + tr + n * C::ROWS_T, zo);
+                epilogue_node<T, EPI>(p, acc, ct.x0 + tx, ct.y0 + tr + n * C::ROWS_T, ct.z0 + i - 2);
             }
         }
-        ++i;
+        if (++s == C::NS) { s = 0; par ^= 1u; }
+        if (++i == ct.nin) {
+            i = 0;
+            item += gridDim.x;
+            if (item < nitems) ct = tma_item<C>(L, p.lz, gx, gy, item);
+        }
     };
 
-    static_assert(C::NS == 3, "stage ring and accumulator rotation share the period 3");
-    uint32_t par = 0;
-    while (true) {
-        plane(a0, a1, a2, 0, par);
-        if (i >= nin) break;
-        plane(a1, a2, a0, 1, par);
-        if (i >= nin) break;
-        plane(a2, a0, a1, 2, par);
-        if (i >= nin) break;
-        par ^= 1u;
+    while (true) {   // accumulator sets rotate with period 3
+        plane(a0, a1, a2);
+        if (item >= nitems) break;
+        plane(a1, a2, a0);
+        if (item >= nitems) break;
+        plane(a2, a0, a1);
+        if (item >= nitems) break;
     }
 }
 

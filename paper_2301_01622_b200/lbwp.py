@@ -14,7 +14,7 @@ import os
 import numpy as np
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_PKG, "liblbwp.so")
+LIB_PATH = os.environ.get("LBWP_LIB") or os.path.join(_PKG, "liblbwp.so")   # LBWP_LIB: another build of the same ABI
 
 LBWP_F32, LBWP_F64 = 0, 1
 LBWP_MOMENTS, LBWP_POPULATIONS = 0, 1
