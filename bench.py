@@ -168,6 +168,18 @@ def run_reference(a):
     print(json.dumps(line))
 
 
+def max_over_ranks(x, world, device="cpu"):
+    """MAX all-reduce of one float over the ranks (nccl on the GPU box, gloo in the CPU test)."""
+    if world == 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([x], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def aggregate(per_rank_nodes_steps, max_ms):
     """value over all ranks: total node updates / max-over-ranks time (host logic; gloo-tested)."""
     return sum(per_rank_nodes_steps) / (max_ms * 1e-3) / 1e6
@@ -222,10 +234,7 @@ def main():
     barrier()
     clocks = sampler.stop()
     ms = ev0.elapsed_time(ev1)
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, world, "cuda")
     value = aggregate([nodes * a.steps] * world, ms)
 
     # end-to-end through the C ABI with HOST buffers: every step uploads the state from pinned host
@@ -247,10 +256,7 @@ def main():
             h_in, h_out = h_out, h_in
         barrier()
         dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dt, world, "cuda")
         nbytes = h_in.numel() * h_in.element_size()
         e2e = {"value": nodes * a.e2e_steps * world / dt / 1e6, "unit": METRIC, "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes, "steps": a.e2e_steps,

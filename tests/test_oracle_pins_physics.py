@@ -73,3 +73,81 @@ def test_sound_speed(oracle, q):
     t_zero = i + amps[i - 1] / (amps[i - 1] - amps[i])  # linear interpolation, time of step index i-1 is i
     cs = math.pi / (2 * k * t_zero)
     assert abs(cs * math.sqrt(3) - 1) < 0.01
+
+
+# ---- two-component step (reading C6): invariants the mathematics fixes -------------------
+def _droplet_state(n=20, seed=3):
+    cfg = wl.config3(n)
+    m = np.array(cfg["moments"], dtype=np.float64)
+    rng = np.random.default_rng(seed)
+    m[2:5] += 0.01 * rng.uniform(-1, 1, m[2:5].shape)            # some flow everywhere
+    m[5:] += 1e-3 * rng.uniform(-1, 1, m[5:].shape)              # off-equilibrium Pi
+    return m
+
+
+# P10: with A = 0 the recolouring leaves the total populations untouched, so the total fluid evolves
+#      exactly as the single-component scheme from the same total fields, for any beta.
+@pytest.mark.parametrize("q", LATTICES)
+@pytest.mark.parametrize("beta", [0.0, 0.7])
+def test_two_component_A0_reduces_to_single(oracle, q, beta):
+    m2 = _droplet_state()
+    m1 = np.concatenate([(m2[0] + m2[1])[None], m2[2:]])
+    o2 = oracle.run(m2, lattice=q, ncomp=2, tau=0.8, nsteps=6, A=0.0, beta=beta)
+    o1 = oracle.run(m1, lattice=q, ncomp=1, tau=0.8, nsteps=6)
+    assert np.abs((o2[0] + o2[1]) - o1[0]).max() < 1e-13
+    assert np.abs(o2[2:] - o1[1:]).max() < 1e-13
+
+
+# P11: each colour's mass and the total momentum are conserved (perturbation has zero mass and
+#      momentum, sum_i w_i cos(theta_i) = 0), with surface tension and recolouring switched on.
+@pytest.mark.parametrize("q", LATTICES)
+def test_two_component_conservation(oracle, q):
+    m = _droplet_state()
+    o = oracle.run(m, lattice=q, ncomp=2, tau=1.0, nsteps=8, A=0.01, beta=0.7)
+    for k in (0, 1):
+        assert abs(o[k].sum() - m[k].sum()) < 1e-10
+    for a in range(3):
+        p0 = ((m[0] + m[1]) * m[2 + a]).sum()
+        p1 = ((o[0] + o[1]) * o[2 + a]).sum()
+        assert abs(p1 - p0) < 1e-11
+    assert np.abs(o - oracle.run(m, lattice=q, ncomp=2, tau=1.0, nsteps=8, A=0.0, beta=0.7)).max() > 1e-6  # A acts
+
+
+# beta = 0, A = 0: both colours are passive copies of the total fluid: rhoA / rho is simply advected
+# and a uniform mixture stays uniform.
+def test_two_component_uniform_mixture_is_fixed_point(oracle):
+    shape = (6, 5, 7)
+    rho_a, rho_b = np.full(shape, 0.3), np.full(shape, 0.7)
+    u = [np.full(shape, 0.02), np.full(shape, -0.01), np.full(shape, 0.03)]
+    m = wl.pack2(rho_a, rho_b, u)
+    o = oracle.run(m, lattice=27, ncomp=2, tau=0.9, nsteps=5, A=0.01, beta=0.7)   # G = 0: no colour terms
+    assert np.abs(o - m).max() < 1e-14
+
+
+# P13 (qualitative): recolouring sharpens a flat interface to a tanh of width ~ 1/beta and keeps it there.
+def test_two_component_interface_stays_sharp(oracle):
+    n = 32
+    x = np.arange(n)
+    phi = np.tanh((8 - np.abs(x - n / 2 + 0.5)) / 2.0)[None, None, :] * np.ones((1, 1, n))
+    m = wl.pack2((1 + phi) / 2, (1 - phi) / 2, [np.zeros_like(phi)] * 3)
+    o = oracle.run(m, lattice=27, ncomp=2, tau=1.0, nsteps=400, A=0.0, beta=0.7)
+    phi1 = (o[0] - o[1]) / (o[0] + o[1])
+    assert phi1[0, 0, n // 2] > 0.99 and phi1[0, 0, 0] < -0.99          # phases stay separated
+    width = np.sum(np.abs(phi1[0, 0, : n // 2]) < 0.76)                 # nodes inside |phi| < tanh(1)
+    assert 1 <= width <= 4                                              # interface a few nodes wide
+    assert abs(o[0].sum() - m[0].sum()) < 1e-10
+
+
+# ---- comparison kernel's mini-oracle (population-storing BGK): conservation + viscosity ------
+@pytest.mark.parametrize("q", LATTICES)
+def test_population_oracle_conservation_and_viscosity(oracle, q):
+    n, tau = 32, 0.8
+    m0 = wl.taylor_green(n, shape=(n, n, 1))
+    m20 = oracle.pop_run(m0, lattice=q, tau=tau, nsteps=20)
+    m100 = oracle.pop_run(m20, lattice=q, tau=tau, nsteps=80)   # restart from moments: Pi^neq re-regularised once
+    assert abs(m100[0].sum() - m0[0].sum()) < 1e-10
+    for a in range(3):
+        assert abs((m100[0] * m100[1 + a]).sum() - (m0[0] * m0[1 + a]).sum()) < 1e-12
+    k = 2 * math.pi / n
+    nu_meas = -math.log(tg_amplitude(m100, n) / tg_amplitude(m20, n)) / (2 * k * k * 80)
+    assert abs(nu_meas / ((tau - 0.5) / 3.0) - 1) < 0.01
