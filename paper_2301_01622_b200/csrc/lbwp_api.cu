@@ -58,7 +58,7 @@ int state_fields(const lbwp_params* p) {
 
 
 bool tma_eligible(const lbwp_params* p) {
-    if (!(p->scheme == LBWP_MOMENTS && p->ncomp == 1 && p->lattice == 27)) return false;
+    if (!(p->scheme == LBWP_MOMENTS && p->ncomp == 1)) return false;
     return p->dtype == LBWP_F32 ? lbwp::tma_eligible_f32(p->nx, p->ny) : lbwp::tma_eligible_f64(p->nx, p->ny);
 }
 
@@ -185,7 +185,7 @@ struct TmaCtx final : lbwp_ctx {
     ~TmaCtx() override { delete planp; }
 
     int prepare() {
-        planp = lbwp::make_tma_plan<T>(X.nx, X.ny);
+        planp = lbwp::make_tma_plan<T>(X.nx, X.ny, P.lattice);
         if (!planp) return fail(LBWP_ENOMEM, "no TMA plan");
         int rc = planp->setup(X, buf);
         if (rc) return fail(rc < 0 ? LBWP_EUNSUPPORTED : LBWP_ECUDA, "TMA plan setup failed (%d): %s", rc,
@@ -203,7 +203,8 @@ struct TmaCtx final : lbwp_ctx {
         const dim3 b(32, 8, 1), g((X.nx + 31) / 32, (X.ny + 7) / 8, X.nz);
         steps = 0;
         cur = 0;
-        lbwp::k_tma_import<T><<<g, b, 0, stream>>>(X, (const T*)ext, (T*)buf[0], (T*)buf[1], T(1.0 / P.tau));
+        if (P.lattice == 27) lbwp::k_tma_import<T, 27><<<g, b, 0, stream>>>(X, (const T*)ext, (T*)buf[0], (T*)buf[1], T(1.0 / P.tau));
+        else lbwp::k_tma_import<T, 19><<<g, b, 0, stream>>>(X, (const T*)ext, (T*)buf[0], (T*)buf[1], T(1.0 / P.tau));
         CU(cudaGetLastError());
         return LBWP_OK;
     }
@@ -263,7 +264,7 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
         return fail(LBWP_EUNSUPPORTED, "population-storing comparison kernel is built for ncomp == 1 only");
     const int variant = choose_variant(p);
     if (variant == 0)
-        return fail(LBWP_EUNSUPPORTED, "kernel %d is not built for this combination (MARCH/TMA: D3Q27 single-component "
+        return fail(LBWP_EUNSUPPORTED, "kernel %d is not built for this combination (MARCH: D3Q27 single-component; TMA: single-component "
                     "moments; TMA also needs nx %% 64 (fp32) or 32 (fp64) == 0 and ny %% 8 == 0)", p->kernel);
     int ndev = 0;
     CU(cudaGetDeviceCount(&ndev));

@@ -12,7 +12,7 @@ namespace lbwp {
 // ---- pointwise conversions (lbwp_init / lbwp_set_moments / lbwp_moments at t = 0; not per step) ----
 // ext: dense [10][nz][ny][nx] moments (include/lbwp.h) -> sform: XLayout S-form (x ghosts included),
 // raw: XLayout copy of the moments themselves (what lbwp_moments returns while no step was taken).
-template <typename T>
+template <typename T, int Q>
 __global__ void __launch_bounds__(256) k_tma_import(XLayout L, const T* __restrict__ ext, T* __restrict__ sform,
                                                     T* __restrict__ raw, T omega) {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
@@ -33,7 +33,7 @@ __global__ void __launch_bounds__(256) k_tma_import(XLayout L, const T* __restri
     for (int k = 0; k < 3; ++k) a[7 + k] = m[7 + k];
     TmaStepParams<T> p;
     p.L = L; p.dst = sform; p.omega = omega; p.lz = 0;
-    epilogue_node<T, EPI_SFORM>(p, a, x, y, z);
+    epilogue_node<T, EPI_SFORM, Q>(p, a, x, y, z);
 }
 
 template <typename T>
@@ -128,7 +128,7 @@ struct TmaPlanT final : TmaPlanBase {
 
     int setup(const XLayout& L_, void* const buf[2]) override {
         L = L_;
-        snprintf(tag, sizeof(tag), "%dx%dx%d_s%d", C::TX, C::TY, C::NPT, C::NS);
+        snprintf(tag, sizeof(tag), "q%d_%dx%dx%d_s%d", C::Q, C::TX, C::TY, C::NPT, C::NS);
         for (int k = 0; k < 2; ++k) {
             int rc = make_state_map<T>(&main_map[k], buf[k], L, C::BW, C::TY);
             if (rc) return rc;
@@ -180,14 +180,18 @@ struct TmaPlanT final : TmaPlanBase {
 
 // first geometry of the dtype's list whose tile divides the box; nullptr if none does
 template <typename T>
-inline TmaPlanBase* make_tma_plan(int nx, int ny);
-#define LBWP_TRY(NPT, TX, TY, NS, MINB) \
-    if (nx % TX == 0 && ny % TY == 0) return new (std::nothrow) TmaPlanT<float, TmaCfg<float, NPT, TX, TY, NS>, MINB>();
-template <> inline TmaPlanBase* make_tma_plan<float>(int nx, int ny) { LBWP_F32_LIST(LBWP_TRY) return nullptr; }
+inline TmaPlanBase* make_tma_plan(int nx, int ny, int q);
+#define LBWP_TRY(NPT, TX, TY, NS, MINB)                                                                      \
+    if (nx % TX == 0 && ny % TY == 0)                                                                        \
+        return q == 27 ? (TmaPlanBase*)new (std::nothrow) TmaPlanT<float, TmaCfg<float, NPT, TX, TY, NS, 27>, MINB>() \
+                       : (TmaPlanBase*)new (std::nothrow) TmaPlanT<float, TmaCfg<float, NPT, TX, TY, NS, 19>, MINB>();
+template <> inline TmaPlanBase* make_tma_plan<float>(int nx, int ny, int q) { LBWP_F32_LIST(LBWP_TRY) return nullptr; }
 #undef LBWP_TRY
-#define LBWP_TRY(NPT, TX, TY, NS, MINB) \
-    if (nx % TX == 0 && ny % TY == 0) return new (std::nothrow) TmaPlanT<double, TmaCfg<double, NPT, TX, TY, NS>, MINB>();
-template <> inline TmaPlanBase* make_tma_plan<double>(int nx, int ny) { LBWP_F64_LIST(LBWP_TRY) return nullptr; }
+#define LBWP_TRY(NPT, TX, TY, NS, MINB)                                                                      \
+    if (nx % TX == 0 && ny % TY == 0)                                                                        \
+        return q == 27 ? (TmaPlanBase*)new (std::nothrow) TmaPlanT<double, TmaCfg<double, NPT, TX, TY, NS, 27>, MINB>() \
+                       : (TmaPlanBase*)new (std::nothrow) TmaPlanT<double, TmaCfg<double, NPT, TX, TY, NS, 19>, MINB>();
+template <> inline TmaPlanBase* make_tma_plan<double>(int nx, int ny, int q) { LBWP_F64_LIST(LBWP_TRY) return nullptr; }
 #undef LBWP_TRY
 #define LBWP_TRY(NPT, TX, TY, NS, MINB) if (nx % TX == 0 && ny % TY == 0) return true;
 inline bool tma_eligible_f32(int nx, int ny) { LBWP_F32_LIST(LBWP_TRY) return false; }

@@ -5,9 +5,9 @@
 namespace lbwp {
 
 // Epilogue of one finished output node.  acc = (drho, j, dP_aa = P_aa - 1/3, P_ab), Eq. 1-3.
-//   EPI_SFORM:   BGK collision in moment space (Eq. 8), store the S-form scaled by 1/216
+//   EPI_SFORM:   BGK collision in moment space (Eq. 8), store the S-form scaled by 1/216 (D3Q19: 1/36)
 //   EPI_MOMENTS: store rho, u = j / rho (reading C11), P  (external dense layout)
-template <typename T, int EPI>
+template <typename T, int EPI, int Q = 27>
 __device__ __forceinline__ void epilogue_node(const TmaStepParams<T>& p, const T (&a)[10], int x, int y, int z) {
     const XLayout& L = p.L;
     const T rho = T(1) + a[0];
@@ -22,7 +22,7 @@ __device__ __forceinline__ void epilogue_node(const TmaStepParams<T>& p, const T
         d[7 * n] = a[7]; d[8 * n] = a[8]; d[9 * n] = a[9];
         return;
     }
-    const T c = T(1.0 / 216.0);
+    const T c = Q == 27 ? T(1.0 / 216.0) : T(1.0 / 36.0);   // common denominator of the lattice weights
     const T om1 = T(1) - p.omega;
     const T wx = p.omega * a[1], wy = p.omega * a[2], wz = p.omega * a[3];   // omega rho u
     const T iso = a[0] * T(1.0 / 3.0);                                        // rho cs^2 - 1/3
@@ -45,6 +45,44 @@ __device__ __forceinline__ void epilogue_node(const TmaStepParams<T>& p, const T
     out[9] = (T(9) * c) * syz;
     const long long F = L.field;
     T* __restrict__ d = p.dst + xidx(L, x, y, z);
+#pragma unroll
+    for (int f = 0; f < 10; ++f) d[f * F] = out[f];
+    if (x == 0 || x == L.nx - 1) {   // periodic image in the x ghost column (reading C13); nx >= 2 here
+        T* __restrict__ g = x == 0 ? d + L.nx : d - L.nx;
+#pragma unroll
+        for (int f = 0; f < 10; ++f) g[f * F] = out[f];
+    }
+}
+
+// The same collision over all nodes a thread owns at once (packed FMUL2/FFMA2 for the fp32 pair), and
+// the stores of one node of the result.
+template <typename T, typename V, int N, int Q>
+__device__ __forceinline__ void collide_sform_v(const V (&a)[10], T omega, V (&out)[10]) {
+    const T c = Q == 27 ? T(1.0 / 216.0) : T(1.0 / 36.0);
+    V irho;
+#pragma unroll
+    for (int n = 0; n < N; ++n) irho.set(n, rcp_t<T>(T(1) + a[0].get(n)));
+    const V om = V::bc(omega), om1 = V::bc(T(1) - omega);
+    const V ux = a[1] * irho, uy = a[2] * irho, uz = a[3] * irho;
+    const V wx = om * a[1], wy = om * a[2], wz = om * a[3];          // omega rho u
+    const V iso = a[0] * V::bc(T(1.0 / 3.0));                        // rho cs^2 - 1/3
+    const V sxx = vfma(wx, ux, om1 * (a[4] - iso));
+    const V syy = vfma(wy, uy, om1 * (a[5] - iso));
+    const V szz = vfma(wz, uz, om1 * (a[6] - iso));
+    const V sxy = vfma(wx, uy, om1 * a[7]);
+    const V sxz = vfma(wx, uz, om1 * a[8]);
+    const V syz = vfma(wy, uz, om1 * a[9]);
+    out[0] = V::bc(c) * vfma(V::bc(T(-1.5)), sxx + syy + szz, a[0]);
+    const V c3 = V::bc(T(3) * c), c45 = V::bc(T(4.5) * c), c9 = V::bc(T(9) * c);
+    out[1] = c3 * a[1]; out[2] = c3 * a[2]; out[3] = c3 * a[3];
+    out[4] = c45 * sxx; out[5] = c45 * syy; out[6] = c45 * szz;
+    out[7] = c9 * sxy; out[8] = c9 * sxz; out[9] = c9 * syz;
+}
+
+template <typename T>
+__device__ __forceinline__ void store_sform_node(const XLayout& L, T* __restrict__ dst, const T (&out)[10], int x, int y, int z) {
+    const long long F = L.field;
+    T* __restrict__ d = dst + xidx(L, x, y, z);
 #pragma unroll
     for (int f = 0; f < 10; ++f) d[f * F] = out[f];
     if (x == 0 || x == L.nx - 1) {   // periodic image in the x ghost column (reading C13); nx >= 2 here
@@ -175,17 +213,33 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
             P[f] = P[f] + Cc[f];
         }
 #else
-        S::consume(sm, rs, P, Cc, N);
+        if (C::Q == 27) S::consume(sm, rs, P, Cc, N);
+        else S::consume19(sm, rs, P, Cc, N);
 #endif
         __syncwarp();
         if ((tid & 31) == 0) mbar_arrive(empty(s));
         if (i >= 2) {                               // this input plane completes output plane z0 + i - 2
+            // collision over the thread's nodes at once, except where it costs registers the stencil needs
+            // (fp32 D3Q27 at 96 registers: packed epilogue spills and measured 56 vs 62 GLUPS)
+            constexpr bool kVectorEpilogue = !(C::Q == 27 && C::NPT == 2);
+            if (EPI == EPI_SFORM && kVectorEpilogue) {
+                V out[10];
+                collide_sform_v<T, V, C::NPT, C::Q>(P, p.omega, out);
 #pragma unroll
-            for (int n = 0; n < C::NPT; ++n) {
-                T acc[10];
+                for (int n = 0; n < C::NPT; ++n) {
+                    T o[10];
 #pragma unroll
-                for (int f = 0; f < 10; ++f) acc[f] = P[f].get(n);
-                epilogue_node<T, EPI>(p, acc, ct.x0 + tx, ct.y0 + tr + n * C::ROWS_T, ct.z0 + i - 2);
+                    for (int f = 0; f < 10; ++f) o[f] = out[f].get(n);
+                    store_sform_node<T>(L, p.dst, o, ct.x0 + tx, ct.y0 + tr + n * C::ROWS_T, ct.z0 + i - 2);
+                }
+            } else {
+#pragma unroll
+                for (int n = 0; n < C::NPT; ++n) {
+                    T acc[10];
+#pragma unroll
+                    for (int f = 0; f < 10; ++f) acc[f] = P[f].get(n);
+                    epilogue_node<T, EPI, C::Q>(p, acc, ct.x0 + tx, ct.y0 + tr + n * C::ROWS_T, ct.z0 + i - 2);
+                }
             }
         }
         if (++s == C::NS) { s = 0; par ^= 1u; }

@@ -15,9 +15,10 @@ struct TmaStepParams {
 };
 
 // Compile-time geometry of one instance.
-template <typename T, int NPT_, int TX_, int TY_, int NS_>
+template <typename T, int NPT_, int TX_, int TY_, int NS_, int Q_ = 27>
 struct TmaCfg {
-    static constexpr int NPT = NPT_, TX = TX_, TY = TY_, NS = NS_, M = 10;
+    static constexpr int NPT = NPT_, TX = TX_, TY = TY_, NS = NS_, M = 10, Q = Q_;
+    static_assert(Q_ == 27 || Q_ == 19, "lattice");
     static constexpr int OX = 16 / (int)sizeof(T);            // halo column sits at OX-1 and OX+TX
     static constexpr int BW = TX + 2 * OX;                    // box width: 16-byte multiple
     static constexpr int ROW = M * BW;                        // elements per tile row [field][BW]
@@ -74,37 +75,48 @@ struct TmaStep {
         return v;
     }
 
-    // brackets of one source row (cy = CY): E, W = E + Szz, O at cx = -1, 0, +1, then the x-pass
-    template <int CY>
-    __device__ static __forceinline__ void row(const T* __restrict__ s, const int (&r)[C::NPT][3], const V& four,
-                                               XRow<V>& re, XRow<V>& rw, XRow<V>& ro) {
+    // brackets of one source row (cy = CY) at cx = -1, 0, +1: E, W = E + Szz, O.  WO = false skips the
+    // z-dependent parts where the lattice has no direction (D3Q19: cz != 0 and cx cy != 0).
+    template <int CY, bool WO_CORNERS>
+    __device__ static __forceinline__ void brackets(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&E)[3],
+                                                    V (&W)[3], V (&O)[3]) {
         constexpr int J = 1 - CY;  // row slot of source y - cy: slot 0 = y-1, 1 = y, 2 = y+1
-        V E[3], W[3], O[3];
 #pragma unroll
         for (int cx = -1; cx <= 1; ++cx) {
+            const bool wo = WO_CORNERS || cx == 0 || CY == 0;
             V e, o, z;
-            if (cx == -1) { e = ld<0, -1>(s, r, J); o = ld<3, -1>(s, r, J); z = ld<6, -1>(s, r, J);
-                            e = e + ld<4, -1>(s, r, J); e = e - ld<1, -1>(s, r, J); o = o - ld<8, -1>(s, r, J); }
-            if (cx == 0) { e = ld<0, 0>(s, r, J); o = ld<3, 0>(s, r, J); z = ld<6, 0>(s, r, J); }
-            if (cx == 1) { e = ld<0, 1>(s, r, J); o = ld<3, 1>(s, r, J); z = ld<6, 1>(s, r, J);
-                           e = e + ld<4, 1>(s, r, J); e = e + ld<1, 1>(s, r, J); o = o + ld<8, 1>(s, r, J); }
+            if (cx == -1) { e = ld<0, -1>(s, r, J); e = e + ld<4, -1>(s, r, J); e = e - ld<1, -1>(s, r, J);
+                            if (wo) { o = ld<3, -1>(s, r, J); z = ld<6, -1>(s, r, J); o = o - ld<8, -1>(s, r, J); } }
+            if (cx == 0) { e = ld<0, 0>(s, r, J);
+                           if (wo) { o = ld<3, 0>(s, r, J); z = ld<6, 0>(s, r, J); } }
+            if (cx == 1) { e = ld<0, 1>(s, r, J); e = e + ld<4, 1>(s, r, J); e = e + ld<1, 1>(s, r, J);
+                           if (wo) { o = ld<3, 1>(s, r, J); z = ld<6, 1>(s, r, J); o = o + ld<8, 1>(s, r, J); } }
             if (CY != 0) {
-                V syy, jy, syz;
-                if (cx == -1) { syy = ld<5, -1>(s, r, J); jy = ld<2, -1>(s, r, J); syz = ld<9, -1>(s, r, J); }
-                if (cx == 0) { syy = ld<5, 0>(s, r, J); jy = ld<2, 0>(s, r, J); syz = ld<9, 0>(s, r, J); }
-                if (cx == 1) { syy = ld<5, 1>(s, r, J); jy = ld<2, 1>(s, r, J); syz = ld<9, 1>(s, r, J); }
+                V syy, jy;
+                if (cx == -1) { syy = ld<5, -1>(s, r, J); jy = ld<2, -1>(s, r, J); }
+                if (cx == 0) { syy = ld<5, 0>(s, r, J); jy = ld<2, 0>(s, r, J); }
+                if (cx == 1) { syy = ld<5, 1>(s, r, J); jy = ld<2, 1>(s, r, J); }
                 e = e + syy;
                 e = CY > 0 ? e + jy : e - jy;
-                o = CY > 0 ? o + syz : o - syz;
+                if (wo) {
+                    V syz = cx == -1 ? ld<9, -1>(s, r, J) : cx == 0 ? ld<9, 0>(s, r, J) : ld<9, 1>(s, r, J);
+                    o = CY > 0 ? o + syz : o - syz;
+                }
                 if (cx != 0) {
                     V sxy = cx == -1 ? ld<7, -1>(s, r, J) : ld<7, 1>(s, r, J);
                     e = (cx * CY > 0) ? e + sxy : e - sxy;
                 }
             }
             E[cx + 1] = e;
-            W[cx + 1] = e + z;
-            O[cx + 1] = o;
+            if (wo) { W[cx + 1] = e + z; O[cx + 1] = o; }
         }
+    }
+
+    template <int CY>
+    __device__ static __forceinline__ void row(const T* __restrict__ s, const int (&r)[C::NPT][3], const V& four,
+                                               XRow<V>& re, XRow<V>& rw, XRow<V>& ro) {
+        V E[3], W[3], O[3];
+        brackets<CY, true>(s, r, E, W, O);
         re = xpass<V>(E[0], E[1], E[2], four);
         rw = xpass<V>(W[0], W[1], W[2], four);
         ro = xpass<V>(O[0], O[1], O[2], four);
@@ -139,6 +151,38 @@ struct TmaStep {
         P[0] = P[0] + n00; P[1] = P[1] + n10; P[2] = P[2] + n01; P[3] = P[3] - n00;
         P[4] = P[4] + (mw.m20 - mo.m20); P[5] = P[5] + (mw.m02 - mo.m02); P[6] = P[6] + n00;
         P[7] = P[7] + (mw.m11 - mo.m11); P[8] = P[8] - n10; P[9] = P[9] - n01;
+    }
+
+    // D3Q19 (the paper's lattice): weights x 36 are 12 (rest), 2 (axis), 1 (face diagonal).
+    // In-plane (cz = 0): (1,2,1) x (1,2,1) plus 8 on the centre; off-plane (cz = +-1): a plus shape,
+    // 2 on the centre and 1 on the four in-plane axis neighbours.  Fields are pre-scaled by 1/36.
+    __device__ static __forceinline__ void consume19(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[10],
+                                                     V (&Cc)[10], V (&N)[10]) {
+        const V two = V::bc(T(2)), eight = V::bc(T(8));
+        V El[3], Wl[3], Ol[3], Em[3], Wm[3], Om[3], Eh[3], Wh[3], Oh[3];
+        brackets<-1, false>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
+        brackets<1, false>(s, r, Eh, Wh, Oh);    // sources at y-1 (cy = +1)
+        brackets<0, false>(s, r, Em, Wm, Om);
+        // cz = 0: separable (1,2,1) passes over E, then the extra centre weight
+        const XRow<V> xl = xpass<V>(El[0], El[1], El[2], two), xm = xpass<V>(Em[0], Em[1], Em[2], two),
+                      xh = xpass<V>(Eh[0], Eh[1], Eh[2], two);
+        Mom6<V> me = ypass<V>(xl, xm, xh, two);
+        me.m00 = vfma(eight, Em[1], me.m00);
+        Cc[0] = Cc[0] + me.m00; Cc[1] = Cc[1] + me.m10; Cc[2] = Cc[2] + me.m01;
+        Cc[4] = Cc[4] + me.m20; Cc[5] = Cc[5] + me.m02; Cc[7] = Cc[7] + me.m11;
+        // cz = +-1: plus-shaped moments of B = W + cz O over (0,0), (+-1,0), (0,+-1)
+        const V wx = Wm[2] + Wm[0], wy = Wh[1] + Wl[1], ox = Om[2] + Om[0], oy = Oh[1] + Ol[1];
+        const V w00 = vfma(two, Wm[1], wx + wy), o00 = vfma(two, Om[1], ox + oy);
+        const V w10 = Wm[2] - Wm[0], o10 = Om[2] - Om[0];
+        const V w01 = Wh[1] - Wl[1], o01 = Oh[1] - Ol[1];
+        const V p00 = w00 + o00, p10 = w10 + o10, p01 = w01 + o01;
+        N[0] = p00; N[1] = p10; N[2] = p01; N[3] = p00;
+        N[4] = wx + ox; N[5] = wy + oy; N[6] = p00;
+        N[7] = V::bc(T(0)); N[8] = p10; N[9] = p01;
+        const V n00 = w00 - o00, n10 = w10 - o10, n01 = w01 - o01;
+        P[0] = P[0] + n00; P[1] = P[1] + n10; P[2] = P[2] + n01; P[3] = P[3] - n00;
+        P[4] = P[4] + (wx - ox); P[5] = P[5] + (wy - oy); P[6] = P[6] + n00;
+        P[8] = P[8] - n10; P[9] = P[9] - n01;
     }
 };
 

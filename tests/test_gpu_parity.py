@@ -122,9 +122,11 @@ def test_config2_ragged(lbwp, oracle, dtype, lattice, kernel):
                                          ("f32", (192, 40, 3)), ("f64", (64, 24, 21)), ("f64", (32, 8, 1)),
                                          ("f64", (96, 16, 2))])
 @pytest.mark.parametrize("steps", [1, 2, 25])
-def test_tma_kernel_shapes(lbwp, oracle, dtype, shape, steps):
-    cfg = dict(name="tma_%s_%s" % (dtype, "x".join(map(str, shape))), moments=wl.noisy_solenoidal(0, shape=shape),
-               lattice=27, ncomp=1, tau=0.6, A=0.0, beta=0.0, dtype=dtype)
+@pytest.mark.parametrize("lattice", [27, 19])
+def test_tma_kernel_shapes(lbwp, oracle, dtype, shape, steps, lattice):
+    cfg = dict(name="tma%d_%s_%s" % (lattice, dtype, "x".join(map(str, shape))),
+               moments=wl.noisy_solenoidal(0, shape=shape), lattice=lattice, ncomp=1, tau=0.6, A=0.0, beta=0.0,
+               dtype=dtype)
     check(lbwp, oracle, cfg, steps, kernel="tma")
 
 
