@@ -15,6 +15,7 @@
 #include "lbwp_march.cuh"
 #include "lbwp_pop.cuh"
 #include "lbwp_tma_host.cuh"
+#include "lbwp_tma2.cuh"
 
 namespace {
 
@@ -58,6 +59,8 @@ int state_fields(const lbwp_params* p) {
 
 
 bool tma_eligible(const lbwp_params* p) {
+    if (p->scheme == LBWP_MOMENTS && p->ncomp == 2 && p->lattice == 27)
+        return p->dtype == LBWP_F32 ? lbwp::Tma2Plan<float>::eligible(p->nx, p->ny) : lbwp::Tma2Plan<double>::eligible(p->nx, p->ny);
     if (!(p->scheme == LBWP_MOMENTS && p->ncomp == 1)) return false;
     return p->dtype == LBWP_F32 ? lbwp::tma_eligible_f32(p->nx, p->ny) : lbwp::tma_eligible_f64(p->nx, p->ny);
 }
@@ -221,6 +224,38 @@ struct TmaCtx final : lbwp_ctx {
     }
 };
 
+// Two-component TMA variant (lbwp_tma2.cuh): buf[0] = S15 scratch, buf[1] = R, the state (12 of 15 fields used).
+template <typename T>
+struct Tma2Ctx final : lbwp_ctx {
+    lbwp::Tma2Plan<T> plan;
+    lbwp::XLayout X;
+
+    int prepare() {
+        int rc = plan.setup(X, buf[0]);
+        if (rc) return fail(rc < 0 ? LBWP_EUNSUPPORTED : LBWP_ECUDA, "two-component TMA plan setup failed (%d)", rc);
+        return LBWP_OK;
+    }
+    int step_once() override {
+        int rc = plan.step((T*)buf[1], (T*)buf[0], 1.0 / P.tau, P.A, P.beta, stream);
+        if (rc) return fail(LBWP_ECUDA, "two-component step launch: %s", cudaGetErrorString((cudaError_t)rc));
+        ++steps;
+        return LBWP_OK;
+    }
+    int import_dense(const void* ext) override {
+        const dim3 b(32, 8, 1), g((X.nx + 31) / 32, (X.ny + 7) / 8, X.nz);
+        steps = 0;
+        lbwp::k_tma2_import<T><<<g, b, 0, stream>>>(X, (const T*)ext, (T*)buf[1]);
+        CU(cudaGetLastError());
+        return LBWP_OK;
+    }
+    int export_dense(void* ext) override {
+        const dim3 b(32, 8, 1), g((X.nx + 31) / 32, (X.ny + 7) / 8, X.nz);
+        lbwp::k_tma2_export<T><<<g, b, 0, stream>>>(X, (const T*)buf[1], (T*)ext);
+        CU(cudaGetLastError());
+        return LBWP_OK;
+    }
+};
+
 size_t dense_bytes(const lbwp_ctx* c) { return (size_t)c->M * c->L.nx * c->L.ny * c->L.nz * c->esize; }
 
 int load_moments(lbwp_ctx* c, const void* moments, int on_device) {
@@ -248,7 +283,7 @@ size_t lbwp_state_bytes(const lbwp_params* p) {
     if (variant == 0) return 0;
     if (variant == LBWP_KERNEL_TMA) {
         const lbwp::XLayout X = lbwp::make_xlayout(p->nx, p->ny, p->nz, elem_bytes(p));
-        return (size_t)10 * (size_t)X.field * (size_t)elem_bytes(p);
+        return (size_t)(p->ncomp == 2 ? 15 : 10) * (size_t)X.field * (size_t)elem_bytes(p);
     }
     const lbwp::Layout L = lbwp::make_layout(p->nx, p->ny, p->nz, elem_bytes(p));
     return (size_t)state_fields(p) * (size_t)L.field * (size_t)elem_bytes(p);
@@ -278,7 +313,10 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
     lbwp_ctx* c = nullptr;
     if (variant == LBWP_KERNEL_TMA) {
         const lbwp::XLayout X = lbwp::make_xlayout(p->nx, p->ny, p->nz, elem_bytes(p));
-        if (p->dtype == LBWP_F32) { auto* t = new (std::nothrow) TmaCtx<float>(); if (t) t->X = X; c = t; }
+        if (p->ncomp == 2) {
+            if (p->dtype == LBWP_F32) { auto* t = new (std::nothrow) Tma2Ctx<float>(); if (t) t->X = X; c = t; }
+            else { auto* t = new (std::nothrow) Tma2Ctx<double>(); if (t) t->X = X; c = t; }
+        } else if (p->dtype == LBWP_F32) { auto* t = new (std::nothrow) TmaCtx<float>(); if (t) t->X = X; c = t; }
         else { auto* t = new (std::nothrow) TmaCtx<double>(); if (t) t->X = X; c = t; }
     } else {
         c = p->dtype == LBWP_F32 ? (lbwp_ctx*)new (std::nothrow) Ctx<float>() : (lbwp_ctx*)new (std::nothrow) Ctx<double>();
@@ -304,7 +342,7 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
             if (e != cudaSuccess) return bail(fail(LBWP_ENOMEM, "cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e)));
         }
     }
-    if (p->scheme == LBWP_MOMENTS && p->ncomp == 2) {
+    if (p->scheme == LBWP_MOMENTS && p->ncomp == 2 && variant != LBWP_KERNEL_TMA) {
         cudaError_t e = cudaMalloc(&c->grad, (size_t)3 * c->L.field * c->esize);
         if (e != cudaSuccess) return bail(fail(LBWP_ENOMEM, "cudaMalloc(grad): %s", cudaGetErrorString(e)));
         c->launches_per_step = 2;
@@ -316,7 +354,12 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
     }
     c->variant = variant;
     if (variant == LBWP_KERNEL_TMA) {
-        rc = p->dtype == LBWP_F32 ? static_cast<TmaCtx<float>*>(c)->prepare() : static_cast<TmaCtx<double>*>(c)->prepare();
+        if (p->ncomp == 2) {
+            rc = p->dtype == LBWP_F32 ? static_cast<Tma2Ctx<float>*>(c)->prepare() : static_cast<Tma2Ctx<double>*>(c)->prepare();
+            c->launches_per_step = 2;
+        } else {
+            rc = p->dtype == LBWP_F32 ? static_cast<TmaCtx<float>*>(c)->prepare() : static_cast<TmaCtx<double>*>(c)->prepare();
+        }
         if (rc) return bail(rc);
     }
     snprintf(c->name, sizeof(c->name), "%s%d_%s%s",

@@ -1,0 +1,180 @@
+// lbwp_tma2.cuh -- two-component colour-gradient runs (reading C6) in the paper's own SPLIT form
+// ("collision ... store post-collision hydro fields ... separate streaming kernel"), with the
+// streaming kernel being the TMA stencil of lbwp_tma*.cuh.
+//
+//   pass A  k_colour_collide (pointwise + 26-neighbour gradient of phi, through L1/L2):
+//           R = (rhoA, drho, j, dP_aa, P_ab, phi)  ->  S15 = (S-form with the perturbation folded in, rA, K, R0)
+//   pass B  k_step_tma27<NC = 2>: linear stencil of S15 (consume2c), raw sums stored back into R.
+//
+// R is the state between steps (12 fields, what lbwp_moments reads); S15 is scratch (15 fields).
+// Algorithmic traffic: A reads 12 + writes 15, B reads 15 + writes 12 fields = 54 x sizeof per node and step
+// (216 B fp32), against the 2 x 11 x sizeof of a fully fused step: the fused version is the round-2 item.
+#pragma once
+#include "lbwp_gather.cuh"
+#include "lbwp_tma_host.cuh"
+
+namespace lbwp {
+
+template <typename T>
+struct Colour2Params {
+    XLayout L;
+    const T* __restrict__ raw;   // 12 fields, XLayout (ghost columns unused: this pass wraps its indices)
+    T* __restrict__ s15;         // 15 fields, XLayout, x ghost columns written here
+    T omega, A, beta;
+};
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_colour_collide(const Colour2Params<T> p) {
+    const XLayout& L = p.L;
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= L.nx || y >= L.ny) return;
+    const long long F = L.field, c0 = xidx(L, x, y, z);
+    const T* __restrict__ r = p.raw;
+    // gradient of the phase field, G = (1/cs^2) sum_i w_i c_i phi(x + c_i)  (reading C6)
+    const int xs[3] = {x == 0 ? L.nx - 1 : x - 1, x, x == L.nx - 1 ? 0 : x + 1};
+    const int ys[3] = {y == 0 ? L.ny - 1 : y - 1, y, y == L.ny - 1 ? 0 : y + 1};
+    const int zs[3] = {z == 0 ? L.nz - 1 : z - 1, z, z == L.nz - 1 ? 0 : z + 1};
+    const T* __restrict__ phi = r + 11 * F;
+    T gx = 0, gy = 0, gz = 0;
+#pragma unroll
+    for (int cz = -1; cz <= 1; ++cz)
+#pragma unroll
+        for (int cy = -1; cy <= 1; ++cy) {
+            const long long row = ((long long)zs[cz + 1] * L.ny + ys[cy + 1]) * L.px + L.ox;
+#pragma unroll
+            for (int cx = -1; cx <= 1; ++cx) {
+                const int n2 = cx * cx + cy * cy + cz * cz;
+                if (n2 == 0) continue;
+                const T w = T(3.0 * lattice_w<27>(n2));
+                const T f = phi[row + xs[cx + 1]];
+                if (cx) gx += T(cx) * w * f;
+                if (cy) gy += T(cy) * w * f;
+                if (cz) gz += T(cz) * w * f;
+            }
+        }
+    const T rhoA = r[c0], drho = r[F + c0];
+    const T rho = T(1) + drho, irho = T(1) / rho;
+    const T jx = r[2 * F + c0], jy = r[3 * F + c0], jz = r[4 * F + c0];
+    SNode<T> n = collide_sform<T>(drho, jx * irho, jy * irho, jz * irho, r[5 * F + c0], r[6 * F + c0], r[7 * F + c0],
+                                  r[8 * F + c0], r[9 * F + c0], r[10 * F + c0], p.omega);
+    const T g2 = gx * gx + gy * gy + gz * gz;
+    const T ig = g2 > T(1e-10) ? rsqrt_t<T>(g2) : T(0);   // reading C8
+    const T g = g2 * ig;
+    const T nx = gx * ig, ny = gy * ig, nz = gz * ig;
+    const T Ag = p.A * g;
+    // perturbation: S_tot = S + (A/9)|G| n n, drho' = drho - (A/3)|G|, rest population + (A/3)|G|
+    n.da -= Ag * T(1.0 / 3.0) + Ag * T(1.5 / 9.0);
+    n.Sxx += T(0.5) * Ag * nx * nx;
+    n.Syy += T(0.5) * Ag * ny * ny;
+    n.Szz += T(0.5) * Ag * nz * nz;
+    n.Sxy += Ag * nx * ny;
+    n.Sxz += Ag * nx * nz;
+    n.Syz += Ag * ny * nz;
+    const T rA = rhoA * irho;
+    const T kappa = p.beta * rA * (rho - rhoA);   // beta rhoA rhoB / rho
+    const T c = T(1.0 / 216.0);
+    T out[15];
+    out[0] = c * n.da;
+    out[1] = c * n.Jx; out[2] = c * n.Jy; out[3] = c * n.Jz;
+    out[4] = c * n.Sxx; out[5] = c * n.Syy; out[6] = c * n.Szz;
+    out[7] = c * n.Sxy; out[8] = c * n.Sxz; out[9] = c * n.Syz;
+    out[10] = rA;
+    out[11] = c * kappa * nx; out[12] = c * kappa * ny; out[13] = c * kappa * nz;
+    out[14] = Ag * T(1.0 / 3.0);
+    T* __restrict__ d = p.s15 + c0;
+#pragma unroll
+    for (int f = 0; f < 15; ++f) d[f * F] = out[f];
+    if (x == 0 || x == L.nx - 1) {   // x ghost column for the TMA boxes of pass B
+        T* __restrict__ gdst = x == 0 ? d + L.nx : d - L.nx;
+#pragma unroll
+        for (int f = 0; f < 15; ++f) gdst[f * F] = out[f];
+    }
+}
+
+// dense external moments [11][nz][ny][nx] (rhoA, rhoB, u, P) <-> R
+template <typename T>
+__global__ void __launch_bounds__(256) k_tma2_import(XLayout L, const T* __restrict__ ext, T* __restrict__ raw) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= L.nx || y >= L.ny) return;
+    const long long n = (long long)L.nx * L.ny * L.nz;
+    const long long e = ((long long)z * L.ny + y) * L.nx + x;
+    const long long F = L.field, c = xidx(L, x, y, z);
+    const double ra = (double)ext[e], rb = (double)ext[n + e];
+    const double rho = ra + rb;
+    raw[c] = T(ra);
+    raw[F + c] = T(rho - 1.0);
+    for (int k = 0; k < 3; ++k) raw[(2 + k) * F + c] = T(rho * (double)ext[(2 + k) * n + e]);
+    for (int k = 0; k < 3; ++k) raw[(5 + k) * F + c] = T((double)ext[(5 + k) * n + e] - 1.0 / 3.0);
+    for (int k = 0; k < 3; ++k) raw[(8 + k) * F + c] = ext[(8 + k) * n + e];
+    raw[11 * F + c] = T((ra - rb) / rho);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_tma2_export(XLayout L, const T* __restrict__ raw, T* __restrict__ ext) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= L.nx || y >= L.ny) return;
+    const long long n = (long long)L.nx * L.ny * L.nz;
+    const long long e = ((long long)z * L.ny + y) * L.nx + x;
+    const long long F = L.field, c = xidx(L, x, y, z);
+    const double ra = (double)raw[c], rho = 1.0 + (double)raw[F + c];
+    ext[e] = T(ra);
+    ext[n + e] = T(rho - ra);
+    for (int k = 0; k < 3; ++k) ext[(2 + k) * n + e] = T((double)raw[(2 + k) * F + c] / rho);   // u = j / rho (C11)
+    for (int k = 0; k < 3; ++k) ext[(5 + k) * n + e] = T((double)raw[(5 + k) * F + c] + 1.0 / 3.0);
+    for (int k = 0; k < 3; ++k) ext[(8 + k) * n + e] = raw[(8 + k) * F + c];
+}
+
+// ---- host side: one two-component plan per dtype ----------------------------------------------------
+template <typename T> struct Tma2Geom;
+template <> struct Tma2Geom<float> { using C = TmaCfg<float, 2, 64, 8, 3, 27, 2>; };
+template <> struct Tma2Geom<double> { using C = TmaCfg<double, 1, 32, 8, 3, 27, 2>; };
+
+template <typename T>
+struct Tma2Plan {
+    using C = typename Tma2Geom<T>::C;
+    XLayout L;
+    CUtensorMap main_map, row_map;   // over the S15 scratch buffer
+    int lz = 0, gz = 0, grid = 0;
+
+    static bool eligible(int nx, int ny) { return nx % C::TX == 0 && ny % C::TY == 0; }
+    static auto kernel() { return k_step_tma27<T, C, EPI_SFORM, 1>; }
+
+    int setup(const XLayout& L_, void* s15) {
+        L = L_;
+        int rc = make_state_map<T>(&main_map, s15, L, C::BW, C::TY, C::M);
+        if (rc) return rc;
+        rc = make_state_map<T>(&row_map, s15, L, C::BW, 1, C::M);
+        if (rc) return rc;
+        cudaError_t e = cudaFuncSetAttribute(kernel(), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+        if (e != cudaSuccess) return (int)e;
+        int per_sm = 0, dev = 0, sms = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel(), C::NT + 32, C::SMEM) != cudaSuccess || per_sm < 1)
+            per_sm = 1;
+        const long long cols = (long long)(L.nx / C::TX) * (L.ny / C::TY);
+        tma_choose_chunks(L.nz, cols, per_sm * sms, &lz, &gz);
+        grid = (int)(cols * gz);
+        return 0;
+    }
+
+    // one time step: collide R -> S15, then stream S15 -> R
+    int step(T* raw, T* s15, double omega, double A, double beta, cudaStream_t stream) const {
+        Colour2Params<T> a;
+        a.L = L; a.raw = raw; a.s15 = s15; a.omega = T(omega); a.A = T(A); a.beta = T(beta);
+        const dim3 b(32, 8, 1), g((L.nx + 31) / 32, (L.ny + 7) / 8, L.nz);
+        k_colour_collide<T><<<g, b, 0, stream>>>(a);
+        TmaStepParams<T> p;
+        p.L = L; p.dst = raw; p.omega = T(omega); p.lz = lz;
+        kernel()<<<grid, C::NT + 32, C::SMEM, stream>>>(main_map, row_map, p);
+        return (int)cudaGetLastError();
+    }
+};
+
+}  // namespace lbwp

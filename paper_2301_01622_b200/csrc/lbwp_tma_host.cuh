@@ -66,15 +66,15 @@ inline PFN_encodeTiled get_encode_tiled() {
     return fn;
 }
 
-// Tensor of one state buffer as TMA sees it: dims (x: px, field: 10, y: ny, z: nz); box (bw, 10, rows, 1).
+// Tensor of one state buffer as TMA sees it: dims (x: px, field: M, y: ny, z: nz); box (bw, M, rows, 1).
 template <typename T>
-inline int make_state_map(CUtensorMap* out, const void* buf, const XLayout& L, int bw, int rows) {
+inline int make_state_map(CUtensorMap* out, const void* buf, const XLayout& L, int bw, int rows, int nfields = 10) {
     PFN_encodeTiled enc = get_encode_tiled();
     if (!enc) return -1;
-    const cuuint64_t dims[4] = {(cuuint64_t)L.px, 10, (cuuint64_t)L.ny, (cuuint64_t)L.nz};
+    const cuuint64_t dims[4] = {(cuuint64_t)L.px, (cuuint64_t)nfields, (cuuint64_t)L.ny, (cuuint64_t)L.nz};
     const cuuint64_t strides[3] = {(cuuint64_t)L.field * sizeof(T), (cuuint64_t)L.px * sizeof(T),
                                    (cuuint64_t)L.plane * sizeof(T)};
-    const cuuint32_t box[4] = {(cuuint32_t)bw, 10, (cuuint32_t)rows, 1};
+    const cuuint32_t box[4] = {(cuuint32_t)bw, (cuuint32_t)nfields, (cuuint32_t)rows, 1};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_128B;
     if (const char* e = getenv("LBWP_TMA_L2PROMO")) promo = (CUtensorMapL2promotion)atoi(e);   // tuning override

@@ -92,6 +92,19 @@ __device__ __forceinline__ void store_sform_node(const XLayout& L, T* __restrict
     }
 }
 
+// Two-component runs (lbwp_tma2.cuh): the finished sums are stored as they are, (rhoA, drho, j, dP_aa,
+// P_ab) plus the phase field phi = (rhoA - rhoB)/rho the next collision pass differentiates.
+template <typename T>
+__device__ __forceinline__ void store_raw2_node(const XLayout& L, T* __restrict__ dst, const T (&a)[11], int x, int y, int z) {
+    const long long F = L.field;
+    T* __restrict__ d = dst + xidx(L, x, y, z);
+    d[0] = a[10];
+#pragma unroll
+    for (int f = 0; f < 10; ++f) d[(1 + f) * F] = a[f];
+    const T rho = T(1) + a[0];
+    d[11 * F] = (a[10] + a[10] - rho) * rcp_t<T>(rho);
+}
+
 // Work decomposition: item = (z chunk, tile row, tile column), x fastest, so that items handled at
 // the same time by neighbouring CTAs are spatial neighbours and their halo reads meet in L2.
 struct TmaItem {
@@ -187,9 +200,9 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
         }
     }
 
-    V a0[10], a1[10], a2[10];
+    V a0[C::NA], a1[C::NA], a2[C::NA];
 #pragma unroll
-    for (int f = 0; f < 10; ++f) a0[f] = a1[f] = a2[f] = V::bc(T(0));
+    for (int f = 0; f < C::NA; ++f) a0[f] = a1[f] = a2[f] = V::bc(T(0));
 
     TmaItem ct = tma_item<C>(L, p.lz, gx, gy, item);
     int i = 0;            // input plane counter within the item
@@ -198,7 +211,7 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
 
     // The first two planes of an item only prime the accumulators (their "finished" planes belong to
     // the z halo and are not stored), so nothing has to be reset at an item boundary.
-    auto plane = [&](V(&P)[10], V(&Cc)[10], V(&N)[10]) {
+    auto plane = [&](V(&P)[C::NA], V(&Cc)[C::NA], V(&N)[C::NA]) {
         int rs[C::NPT][3];
 #pragma unroll
         for (int n = 0; n < C::NPT; ++n)
@@ -213,7 +226,8 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
             P[f] = P[f] + Cc[f];
         }
 #else
-        if (C::Q == 27) S::consume(sm, rs, P, Cc, N);
+        if constexpr (C::NC == 2) S::consume2c(sm, rs, P, Cc, N);
+        else if constexpr (C::Q == 27) S::consume(sm, rs, P, Cc, N);
         else S::consume19(sm, rs, P, Cc, N);
 #endif
         __syncwarp();
@@ -222,9 +236,17 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
             // collision over the thread's nodes at once, except where it costs registers the stencil needs
             // (fp32 D3Q27 at 96 registers: packed epilogue spills and measured 56 vs 62 GLUPS)
             constexpr bool kVectorEpilogue = !(C::Q == 27 && C::NPT == 2);
-            if (EPI == EPI_SFORM && kVectorEpilogue) {
+            if constexpr (C::NC == 2) {
+#pragma unroll
+                for (int n = 0; n < C::NPT; ++n) {
+                    T acc[C::NA];
+#pragma unroll
+                    for (int f = 0; f < C::NA; ++f) acc[f] = P[f].get(n);
+                    store_raw2_node<T>(L, p.dst, acc, ct.x0 + tx, ct.y0 + tr + n * C::ROWS_T, ct.z0 + i - 2);
+                }
+            } else if (EPI == EPI_SFORM && kVectorEpilogue) {
                 V out[10];
-                collide_sform_v<T, V, C::NPT, C::Q>(P, p.omega, out);
+                collide_sform_v<T, V, C::NPT, C::Q>(reinterpret_cast<const V(&)[10]>(P), p.omega, out);
 #pragma unroll
                 for (int n = 0; n < C::NPT; ++n) {
                     T o[10];

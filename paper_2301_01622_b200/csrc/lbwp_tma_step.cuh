@@ -15,10 +15,16 @@ struct TmaStepParams {
 };
 
 // Compile-time geometry of one instance.
-template <typename T, int NPT_, int TX_, int TY_, int NS_, int Q_ = 27>
+// NC = 1: ten S-form fields in, ten out.  NC = 2 (colour gradient, split scheme of lbwp_tma2.cuh): fifteen
+// fields in (S-form with the perturbation folded in, rhoA/rho, the recolouring vector K, the rest-population
+// term), eleven moment sums per node (rhoA added).
+template <typename T, int NPT_, int TX_, int TY_, int NS_, int Q_ = 27, int NC_ = 1>
 struct TmaCfg {
-    static constexpr int NPT = NPT_, TX = TX_, TY = TY_, NS = NS_, M = 10, Q = Q_;
+    static constexpr int NPT = NPT_, TX = TX_, TY = TY_, NS = NS_, Q = Q_, NC = NC_;
+    static constexpr int M = NC_ == 1 ? 10 : 15;      // fields per node in a stage
+    static constexpr int NA = NC_ == 1 ? 10 : 11;     // moment sums per node
     static_assert(Q_ == 27 || Q_ == 19, "lattice");
+    static_assert(NC_ == 1 || Q_ == 27, "the two-component stencil is built for D3Q27");
     static constexpr int OX = 16 / (int)sizeof(T);            // halo column sits at OX-1 and OX+TX
     static constexpr int BW = TX + 2 * OX;                    // box width: 16-byte multiple
     static constexpr int ROW = M * BW;                        // elements per tile row [field][BW]
@@ -124,8 +130,8 @@ struct TmaStep {
 
     // consume one S-form input plane z: last contribution to output plane z-1 (P), middle one to
     // plane z (C), first one to plane z+1 (N, assigned).  Order: rho, jx, jy, jz, pxx, pyy, pzz, pxy, pxz, pyz
-    __device__ static __forceinline__ void consume(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[10],
-                                                   V (&Cc)[10], V (&N)[10]) {
+    __device__ static __forceinline__ void consume(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
+                                                   V (&Cc)[C::NA], V (&N)[C::NA]) {
         const V four = V::bc(T(4));
         XRow<V> el, ew, eo, ml, mw_, mo_, hl, hw, ho;
         row<-1>(s, r, four, el, ew, eo);   // sources at y+1 (cy = -1)
@@ -156,8 +162,8 @@ struct TmaStep {
     // D3Q19 (the paper's lattice): weights x 36 are 12 (rest), 2 (axis), 1 (face diagonal).
     // In-plane (cz = 0): (1,2,1) x (1,2,1) plus 8 on the centre; off-plane (cz = +-1): a plus shape,
     // 2 on the centre and 1 on the four in-plane axis neighbours.  Fields are pre-scaled by 1/36.
-    __device__ static __forceinline__ void consume19(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[10],
-                                                     V (&Cc)[10], V (&N)[10]) {
+    __device__ static __forceinline__ void consume19(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
+                                                     V (&Cc)[C::NA], V (&N)[C::NA]) {
         const V two = V::bc(T(2)), eight = V::bc(T(8));
         V El[3], Wl[3], Ol[3], Em[3], Wm[3], Om[3], Eh[3], Wh[3], Oh[3];
         brackets<-1, false>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
@@ -183,6 +189,88 @@ struct TmaStep {
         P[0] = P[0] + n00; P[1] = P[1] + n10; P[2] = P[2] + n01; P[3] = P[3] - n00;
         P[4] = P[4] + (wx - ox); P[5] = P[5] + (wy - oy); P[6] = P[6] + n00;
         P[8] = P[8] - n10; P[9] = P[9] - n01;
+    }
+
+    // Two-component plane (reading C6; fields as written by k_colour_collide in lbwp_tma2.cuh):
+    //   0..9  S-form of the total fluid with the perturbation folded in     (x 1/216)
+    //   10    rA = rhoA / rho                                                (plain ratio)
+    //   11..13 K = beta rhoA rhoB / rho * n                                  (x 1/216)
+    //   14    R0 = (A/3)|G|, the extra rest population of the perturbation   (population units)
+    // Total moments as in consume(); rhoA (sum 10) gathers the recoloured populations
+    //   hA_c = rA (w_c + h_c) + w_c K.c/|c|      (+ rA R0 for the rest direction).
+    template <int CY>
+    __device__ static __forceinline__ void colour_row(const T* __restrict__ s, const int (&r)[C::NPT][3], const V (&E)[3],
+                                                      const V (&W)[3], const V (&O)[3], const V& four, V& ae, V& aw, V& ao) {
+        constexpr int J = 1 - CY;
+        const V cc = V::bc(T(1.0 / 216.0));
+        const V ra[3] = {ld<10, -1>(s, r, J), ld<10, 0>(s, r, J), ld<10, 1>(s, r, J)};
+        V AE[3], AW[3], AO[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const V rac = ra[k] * cc;
+            AE[k] = vfma(ra[k], E[k], rac);
+            AW[k] = vfma(ra[k], W[k], rac);
+            AO[k] = ra[k] * O[k];
+        }
+        ae = vfma(four, AE[1], AE[2] + AE[0]);   // x-pass, zeroth moment only
+        aw = vfma(four, AW[1], AW[2] + AW[0]);
+        ao = vfma(four, AO[1], AO[2] + AO[0]);
+    }
+
+    __device__ static __forceinline__ void consume2c(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
+                                                     V (&Cc)[C::NA], V (&N)[C::NA]) {
+        const V four = V::bc(T(4));
+        V El[3], Wl[3], Ol[3], Em[3], Wm[3], Om[3], Eh[3], Wh[3], Oh[3];
+        brackets<-1, true>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
+        brackets<1, true>(s, r, Eh, Wh, Oh);    // sources at y-1 (cy = +1)
+        brackets<0, true>(s, r, Em, Wm, Om);
+        {   // total fluid: identical to consume()
+            const Mom6<V> me = ypass<V>(xpass<V>(El[0], El[1], El[2], four), xpass<V>(Em[0], Em[1], Em[2], four),
+                                        xpass<V>(Eh[0], Eh[1], Eh[2], four), four);
+            const Mom6<V> mw = ypass<V>(xpass<V>(Wl[0], Wl[1], Wl[2], four), xpass<V>(Wm[0], Wm[1], Wm[2], four),
+                                        xpass<V>(Wh[0], Wh[1], Wh[2], four), four);
+            const Mom6<V> mo = ypass<V>(xpass<V>(Ol[0], Ol[1], Ol[2], four), xpass<V>(Om[0], Om[1], Om[2], four),
+                                        xpass<V>(Oh[0], Oh[1], Oh[2], four), four);
+            Cc[0] = vfma(four, me.m00, Cc[0]);
+            Cc[1] = vfma(four, me.m10, Cc[1]);
+            Cc[2] = vfma(four, me.m01, Cc[2]);
+            Cc[4] = vfma(four, me.m20, Cc[4]);
+            Cc[5] = vfma(four, me.m02, Cc[5]);
+            Cc[7] = vfma(four, me.m11, Cc[7]);
+            const V p00 = mw.m00 + mo.m00, p10 = mw.m10 + mo.m10, p01 = mw.m01 + mo.m01;
+            N[0] = p00; N[1] = p10; N[2] = p01; N[3] = p00;
+            N[4] = mw.m20 + mo.m20; N[5] = mw.m02 + mo.m02; N[6] = p00;
+            N[7] = mw.m11 + mo.m11; N[8] = p10; N[9] = p01;
+            const V n00 = mw.m00 - mo.m00, n10 = mw.m10 - mo.m10, n01 = mw.m01 - mo.m01;
+            P[0] = P[0] + n00; P[1] = P[1] + n10; P[2] = P[2] + n01; P[3] = P[3] - n00;
+            P[4] = P[4] + (mw.m20 - mo.m20); P[5] = P[5] + (mw.m02 - mo.m02); P[6] = P[6] + n00;
+            P[7] = P[7] + (mw.m11 - mo.m11); P[8] = P[8] - n10; P[9] = P[9] - n01;
+        }
+        // colour A, first part: sum_c w_c rA (1 + B_c)
+        V ael, awl, aol, aem, awm, aom, aeh, awh, aoh;
+        colour_row<-1>(s, r, El, Wl, Ol, four, ael, awl, aol);
+        colour_row<1>(s, r, Eh, Wh, Oh, four, aeh, awh, aoh);
+        colour_row<0>(s, r, Em, Wm, Om, four, aem, awm, aom);
+        const V mae = vfma(four, aem, aeh + ael), maw = vfma(four, awm, awh + awl), mao = vfma(four, aom, aoh + aol);
+        // second part: sum_{c != 0} w_c K.c / |c|; weights x 216 / |c|: 16 (axis), 4/sqrt2 (face), 1/sqrt3 (corner)
+        const V kxa = ld<11, 1>(s, r, 1) - ld<11, -1>(s, r, 1);
+        const V kxb = (ld<11, 1>(s, r, 0) - ld<11, -1>(s, r, 0)) + (ld<11, 1>(s, r, 2) - ld<11, -1>(s, r, 2));
+        const V kya = ld<12, 0>(s, r, 0) - ld<12, 0>(s, r, 2);          // cy = +1 is row slot 0 (source y-1)
+        const V kyb = (ld<12, 1>(s, r, 0) - ld<12, 1>(s, r, 2)) + (ld<12, -1>(s, r, 0) - ld<12, -1>(s, r, 2));
+        const V z0 = ld<13, 0>(s, r, 1);
+        const V z1 = (ld<13, 1>(s, r, 1) + ld<13, -1>(s, r, 1)) + (ld<13, 0>(s, r, 0) + ld<13, 0>(s, r, 2));
+        const V z2 = (ld<13, 1>(s, r, 0) + ld<13, -1>(s, r, 0)) + (ld<13, 1>(s, r, 2) + ld<13, -1>(s, r, 2));
+        const V da = kxa + kya, db = kxb + kyb;
+        const V f1 = V::bc(T(16)), f2 = V::bc(T(2.8284271247461903)), f3 = V::bc(T(0.57735026918962576));
+        const V t0 = vfma(f1, da, f2 * db);                       // cz = 0
+        const V tin = vfma(f2, da, f3 * db);                      // cz = +-1, in-plane part
+        const V tz = vfma(f1, z0, vfma(f2, z1, f3 * z2));         // cz = +-1, c_z K_z part
+        // rest population of the perturbation: to rho and (times rA) to rhoA of the node itself
+        const V r0 = ld<14, 0>(s, r, 1), rac = ld<10, 0>(s, r, 1);
+        Cc[0] = Cc[0] + r0;
+        Cc[10] = vfma(four, mae, Cc[10]) + vfma(rac, r0, t0);
+        N[10] = (maw + mao) + (tin + tz);
+        P[10] = P[10] + ((maw - mao) + (tin - tz));
     }
 };
 
