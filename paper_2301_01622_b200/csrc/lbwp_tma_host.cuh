@@ -128,7 +128,7 @@ struct TmaPlanT final : TmaPlanBase {
 
     int setup(const XLayout& L_, void* const buf[2]) override {
         L = L_;
-        snprintf(tag, sizeof(tag), "q%d_%dx%dx%d_s%d", C::Q, C::TX, C::TY, C::NPT, C::NS);
+        snprintf(tag, sizeof(tag), "q%d_%dx%dx%d_s%d%s", C::Q, C::TX, C::TY, C::NPT, C::NS, C::PX ? "_px" : "");
         for (int k = 0; k < 2; ++k) {
             int rc = make_state_map<T>(&main_map[k], buf[k], L, C::BW, C::TY);
             if (rc) return rc;
@@ -167,33 +167,37 @@ struct TmaPlanT final : TmaPlanBase {
     }
 };
 
+// geometry lists: (nodes per thread, tile x, tile y, stages, min CTAs per SM, x-paired)
 #ifdef LBWP_F32_NPT   // tuning builds: a single fp32 geometry given on the command line
-#define LBWP_F32_LIST(X) X(LBWP_F32_NPT, LBWP_F32_TX, LBWP_F32_TY, LBWP_F32_NS, LBWP_F32_MINB)
+#ifndef LBWP_F32_PX
+#define LBWP_F32_PX 0
+#endif
+#define LBWP_F32_LIST(X) X(LBWP_F32_NPT, LBWP_F32_TX, LBWP_F32_TY, LBWP_F32_NS, LBWP_F32_MINB, LBWP_F32_PX)
 #else
-#define LBWP_F32_LIST(X) X(2, 128, 8, 3, 1) X(2, 64, 8, 3, 1)
+#define LBWP_F32_LIST(X) X(2, 128, 8, 3, 1, 1) X(2, 64, 8, 3, 1, 1)
 #endif
 #ifdef LBWP_F64_NPT
-#define LBWP_F64_LIST(X) X(LBWP_F64_NPT, LBWP_F64_TX, LBWP_F64_TY, LBWP_F64_NS, LBWP_F64_MINB)
+#define LBWP_F64_LIST(X) X(LBWP_F64_NPT, LBWP_F64_TX, LBWP_F64_TY, LBWP_F64_NS, LBWP_F64_MINB, 0)
 #else
-#define LBWP_F64_LIST(X) X(1, 64, 8, 3, 1) X(1, 32, 8, 3, 1)
+#define LBWP_F64_LIST(X) X(1, 64, 8, 3, 1, 0) X(1, 32, 8, 3, 1, 0)
 #endif
 
 // first geometry of the dtype's list whose tile divides the box; nullptr if none does
 template <typename T>
 inline TmaPlanBase* make_tma_plan(int nx, int ny, int q);
-#define LBWP_TRY(NPT, TX, TY, NS, MINB)                                                                      \
+#define LBWP_TRY(NPT, TX, TY, NS, MINB, PX)                                                                  \
     if (nx % TX == 0 && ny % TY == 0)                                                                        \
-        return q == 27 ? (TmaPlanBase*)new (std::nothrow) TmaPlanT<float, TmaCfg<float, NPT, TX, TY, NS, 27>, MINB>() \
-                       : (TmaPlanBase*)new (std::nothrow) TmaPlanT<float, TmaCfg<float, NPT, TX, TY, NS, 19>, MINB>();
+        return q == 27 ? (TmaPlanBase*)new (std::nothrow) TmaPlanT<float, TmaCfg<float, NPT, TX, TY, NS, 27, 1, PX>, MINB>() \
+                       : (TmaPlanBase*)new (std::nothrow) TmaPlanT<float, TmaCfg<float, NPT, TX, TY, NS, 19, 1, PX>, MINB>();
 template <> inline TmaPlanBase* make_tma_plan<float>(int nx, int ny, int q) { LBWP_F32_LIST(LBWP_TRY) return nullptr; }
 #undef LBWP_TRY
-#define LBWP_TRY(NPT, TX, TY, NS, MINB)                                                                      \
+#define LBWP_TRY(NPT, TX, TY, NS, MINB, PX)                                                                  \
     if (nx % TX == 0 && ny % TY == 0)                                                                        \
-        return q == 27 ? (TmaPlanBase*)new (std::nothrow) TmaPlanT<double, TmaCfg<double, NPT, TX, TY, NS, 27>, MINB>() \
-                       : (TmaPlanBase*)new (std::nothrow) TmaPlanT<double, TmaCfg<double, NPT, TX, TY, NS, 19>, MINB>();
+        return q == 27 ? (TmaPlanBase*)new (std::nothrow) TmaPlanT<double, TmaCfg<double, NPT, TX, TY, NS, 27, 1, PX>, MINB>() \
+                       : (TmaPlanBase*)new (std::nothrow) TmaPlanT<double, TmaCfg<double, NPT, TX, TY, NS, 19, 1, PX>, MINB>();
 template <> inline TmaPlanBase* make_tma_plan<double>(int nx, int ny, int q) { LBWP_F64_LIST(LBWP_TRY) return nullptr; }
 #undef LBWP_TRY
-#define LBWP_TRY(NPT, TX, TY, NS, MINB) if (nx % TX == 0 && ny % TY == 0) return true;
+#define LBWP_TRY(NPT, TX, TY, NS, MINB, PX) if (nx % TX == 0 && ny % TY == 0) return true;
 inline bool tma_eligible_f32(int nx, int ny) { LBWP_F32_LIST(LBWP_TRY) return false; }
 inline bool tma_eligible_f64(int nx, int ny) { LBWP_F64_LIST(LBWP_TRY) return false; }
 #undef LBWP_TRY

@@ -92,6 +92,25 @@ __device__ __forceinline__ void store_sform_node(const XLayout& L, T* __restrict
     }
 }
 
+// x-paired fp32 nodes (x, x+1), x even: one 8-byte store per field; ghost images as in store_sform_node
+__device__ __forceinline__ void store_sform_pair(const XLayout& L, float* __restrict__ dst, const f32x2 (&out)[10], int x,
+                                                 int y, int z) {
+    const long long F = L.field;
+    float* __restrict__ d = dst + xidx(L, x, y, z);
+#pragma unroll
+    for (int f = 0; f < 10; ++f) *reinterpret_cast<float2*>(d + f * F) = make_float2(out[f].x, out[f].y);
+    if (x == 0) {
+#pragma unroll
+        for (int f = 0; f < 10; ++f) d[f * F + L.nx] = out[f].x;
+    }
+    if (x + 2 == L.nx) {
+#pragma unroll
+        for (int f = 0; f < 10; ++f) d[f * F - L.nx + 1] = out[f].y;
+    }
+}
+template <typename V>
+__device__ __forceinline__ void store_sform_pair(const XLayout&, double*, const V (&)[10], int, int, int) {}
+
 // Two-component runs (lbwp_tma2.cuh): the finished sums are stored as they are, (rhoA, drho, j, dP_aa,
 // P_ab) plus the phase field phi = (rhoA - rhoB)/rho the next collision pass differentiates.
 template <typename T>
@@ -187,16 +206,19 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
     }
 
     // ---- consumer warps ----
-    const int tx = tid % C::TX, tr = tid / C::TX;
-    // element offsets (within a stage) of the three source rows of each owned node, at x = tx
+    const int tc = tid % C::COLS_T, tr = tid / C::COLS_T;
+    // node n of the thread: column tx + n * DX, row tr + n * DY of the tile
+    constexpr int DX = C::PX ? 1 : 0, DY = C::PX ? 0 : C::ROWS_T;
+    const int tx = C::PX ? 2 * tc : tc;
+    // element offsets (within a stage) of the three source rows of each owned node
     int r[C::NPT][3];
 #pragma unroll
     for (int n = 0; n < C::NPT; ++n) {
-        const int ty = tr + n * C::ROWS_T;
+        const int ty = tr + n * DY;
 #pragma unroll
         for (int j = 0; j < 3; ++j) {
             const int row = ty - 1 + j;
-            r[n][j] = (row < 0 ? C::OFF_YM : row >= C::TY ? C::OFF_YP : row * C::ROW) + C::OX + tx;
+            r[n][j] = (row < 0 ? C::OFF_YM : row >= C::TY ? C::OFF_YP : row * C::ROW) + C::OX + tx + n * DX;
         }
     }
 
@@ -235,24 +257,28 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
         if (i >= 2) {                               // this input plane completes output plane z0 + i - 2
             // collision over the thread's nodes at once, except where it costs registers the stencil needs
             // (fp32 D3Q27 at 96 registers: packed epilogue spills and measured 56 vs 62 GLUPS)
-            constexpr bool kVectorEpilogue = !(C::Q == 27 && C::NPT == 2);
+            constexpr bool kVectorEpilogue = C::PX || !(C::Q == 27 && C::NPT == 2);
             if constexpr (C::NC == 2) {
 #pragma unroll
                 for (int n = 0; n < C::NPT; ++n) {
                     T acc[C::NA];
 #pragma unroll
                     for (int f = 0; f < C::NA; ++f) acc[f] = P[f].get(n);
-                    store_raw2_node<T>(L, p.dst, acc, ct.x0 + tx, ct.y0 + tr + n * C::ROWS_T, ct.z0 + i - 2);
+                    store_raw2_node<T>(L, p.dst, acc, ct.x0 + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
                 }
             } else if (EPI == EPI_SFORM && kVectorEpilogue) {
                 V out[10];
                 collide_sform_v<T, V, C::NPT, C::Q>(reinterpret_cast<const V(&)[10]>(P), p.omega, out);
+                if constexpr (C::PX != 0) {
+                    store_sform_pair(L, p.dst, out, ct.x0 + tx, ct.y0 + tr, ct.z0 + i - 2);
+                } else {
 #pragma unroll
-                for (int n = 0; n < C::NPT; ++n) {
-                    T o[10];
+                    for (int n = 0; n < C::NPT; ++n) {
+                        T o[10];
 #pragma unroll
-                    for (int f = 0; f < 10; ++f) o[f] = out[f].get(n);
-                    store_sform_node<T>(L, p.dst, o, ct.x0 + tx, ct.y0 + tr + n * C::ROWS_T, ct.z0 + i - 2);
+                        for (int f = 0; f < 10; ++f) o[f] = out[f].get(n);
+                        store_sform_node<T>(L, p.dst, o, ct.x0 + tx, ct.y0 + tr + n * DY, ct.z0 + i - 2);
+                    }
                 }
             } else {
 #pragma unroll
@@ -260,7 +286,7 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
                     T acc[10];
 #pragma unroll
                     for (int f = 0; f < 10; ++f) acc[f] = P[f].get(n);
-                    epilogue_node<T, EPI, C::Q>(p, acc, ct.x0 + tx, ct.y0 + tr + n * C::ROWS_T, ct.z0 + i - 2);
+                    epilogue_node<T, EPI, C::Q>(p, acc, ct.x0 + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
                 }
             }
         }

@@ -18,9 +18,13 @@ struct TmaStepParams {
 // NC = 1: ten S-form fields in, ten out.  NC = 2 (colour gradient, split scheme of lbwp_tma2.cuh): fifteen
 // fields in (S-form with the perturbation folded in, rhoA/rho, the recolouring vector K, the rest-population
 // term), eleven moment sums per node (rhoA added).
-template <typename T, int NPT_, int TX_, int TY_, int NS_, int Q_ = 27, int NC_ = 1>
+// PX = 1 (fp32 pairs only): the thread's two nodes are x-adjacent (2t, 2t+1) instead of TY/2 rows apart: one
+// LDS.64 + two LDS.32 bring the four values a field row contributes to both nodes (instead of six LDS.32), and
+// results leave as STG.64.
+template <typename T, int NPT_, int TX_, int TY_, int NS_, int Q_ = 27, int NC_ = 1, int PX_ = 0>
 struct TmaCfg {
-    static constexpr int NPT = NPT_, TX = TX_, TY = TY_, NS = NS_, Q = Q_, NC = NC_;
+    static constexpr int NPT = NPT_, TX = TX_, TY = TY_, NS = NS_, Q = Q_, NC = NC_, PX = PX_;
+    static_assert(PX_ == 0 || (NPT_ == 2 && sizeof(T) == 4 && NC_ == 1), "x-paired mode: fp32, two nodes, one component");
     static constexpr int M = NC_ == 1 ? 10 : 15;      // fields per node in a stage
     static constexpr int NA = NC_ == 1 ? 10 : 11;     // moment sums per node
     static_assert(Q_ == 27 || Q_ == 19, "lattice");
@@ -28,8 +32,9 @@ struct TmaCfg {
     static constexpr int OX = 16 / (int)sizeof(T);            // halo column sits at OX-1 and OX+TX
     static constexpr int BW = TX + 2 * OX;                    // box width: 16-byte multiple
     static constexpr int ROW = M * BW;                        // elements per tile row [field][BW]
-    static constexpr int ROWS_T = TY / NPT;                   // thread rows
-    static constexpr int NT = TX * ROWS_T;
+    static constexpr int ROWS_T = PX_ ? TY : TY / NPT;        // thread rows
+    static constexpr int COLS_T = PX_ ? TX / 2 : TX;          // thread columns
+    static constexpr int NT = COLS_T * ROWS_T;
     static constexpr int NW = NT / 32;
     static constexpr int OFF_YM = TY * ROW;                   // halo row y0-1 (elements)
     static constexpr int OFF_YP = ((((TY + 1) * ROW * (int)sizeof(T)) + 127) / 128) * 128 / (int)sizeof(T);
@@ -122,10 +127,82 @@ struct TmaStep {
     __device__ static __forceinline__ void row(const T* __restrict__ s, const int (&r)[C::NPT][3], const V& four,
                                                XRow<V>& re, XRow<V>& rw, XRow<V>& ro) {
         V E[3], W[3], O[3];
-        brackets<CY, true>(s, r, E, W, O);
+        brackets_any<CY, true>(s, r, E, W, O);
         re = xpass<V>(E[0], E[1], E[2], four);
         rw = xpass<V>(W[0], W[1], W[2], four);
         ro = xpass<V>(O[0], O[1], O[2], four);
+    }
+
+    // ---- x-paired mode (C::PX): r[0][j] is the offset of node 2t in row slot j; node 2t+1 follows it ----
+    // three packed pairs of field F in one source row: hi = sources (x-1, x) for cx = +1, mid = (x, x+1) for
+    // cx = 0, lo = (x+1, x+2) for cx = -1
+    template <int F>
+    __device__ static __forceinline__ void ld3(const T* __restrict__ s, int r0, V& hi, V& mid, V& lo) {
+        const T* __restrict__ q = s + r0 + F * BW;
+        const T lm = q[-1];
+        const float2 c = *reinterpret_cast<const float2*>(q);
+        const T rp = q[2];
+        hi.x = lm; hi.y = c.x;
+        mid.x = c.x; mid.y = c.y;
+        lo.x = c.y; lo.y = rp;
+    }
+    template <int F>
+    __device__ static __forceinline__ V ldm(const T* __restrict__ s, int r0) {
+        const float2 c = *reinterpret_cast<const float2*>(s + r0 + F * BW);
+        V v; v.x = c.x; v.y = c.y;
+        return v;
+    }
+
+    template <int CY, bool WO_CORNERS>
+    __device__ static __forceinline__ void brackets_px(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&E)[3],
+                                                       V (&W)[3], V (&O)[3]) {
+        const int r0 = r[0][1 - CY];
+        const bool wo_side = WO_CORNERS || CY == 0;     // z-dependent parts at cx = +-1
+        V ah, am, al, xh, xm, xl, jh, jm, jl;
+        ld3<0>(s, r0, ah, am, al);
+        ld3<4>(s, r0, xh, xm, xl);                      // Sxx (cx^2)
+        ld3<1>(s, r0, jh, jm, jl);                      // Jx  (cx)
+        E[2] = (ah + xh) + jh;
+        E[1] = am;
+        E[0] = (al + xl) - jl;
+        V zh, zm, zl;
+        if (wo_side) {
+            V oh, om, ol, sh, sm_, sl;
+            ld3<3>(s, r0, oh, om, ol);                  // Jz
+            ld3<6>(s, r0, zh, zm, zl);                  // Szz
+            ld3<8>(s, r0, sh, sm_, sl);                 // Sxz (cx cz)
+            O[2] = oh + sh; O[1] = om; O[0] = ol - sl;
+        } else {
+            O[1] = ldm<3>(s, r0);
+            zm = ldm<6>(s, r0);
+        }
+        if (CY != 0) {
+            V yh, ym, yl, kh, km, kl, ph, pm, pl;
+            ld3<5>(s, r0, yh, ym, yl);                  // Syy (cy^2)
+            ld3<2>(s, r0, kh, km, kl);                  // Jy  (cy)
+            ld3<7>(s, r0, ph, pm, pl);                  // Sxy (cx cy)
+            E[2] = E[2] + yh; E[1] = E[1] + ym; E[0] = E[0] + yl;
+            if (CY > 0) { E[2] = (E[2] + kh) + ph; E[1] = E[1] + km; E[0] = (E[0] + kl) - pl; }
+            else        { E[2] = (E[2] - kh) - ph; E[1] = E[1] - km; E[0] = (E[0] - kl) + pl; }
+            if (wo_side) {
+                V qh, qm, ql;
+                ld3<9>(s, r0, qh, qm, ql);              // Syz (cy cz)
+                if (CY > 0) { O[2] = O[2] + qh; O[1] = O[1] + qm; O[0] = O[0] + ql; }
+                else        { O[2] = O[2] - qh; O[1] = O[1] - qm; O[0] = O[0] - ql; }
+            } else {
+                const V qm = ldm<9>(s, r0);
+                O[1] = CY > 0 ? O[1] + qm : O[1] - qm;
+            }
+        }
+        W[1] = E[1] + zm;
+        if (wo_side) { W[2] = E[2] + zh; W[0] = E[0] + zl; }
+    }
+
+    template <int CY, bool WO_CORNERS>
+    __device__ static __forceinline__ void brackets_any(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&E)[3],
+                                                        V (&W)[3], V (&O)[3]) {
+        if constexpr (C::PX != 0) brackets_px<CY, WO_CORNERS>(s, r, E, W, O);
+        else brackets<CY, WO_CORNERS>(s, r, E, W, O);
     }
 
     // consume one S-form input plane z: last contribution to output plane z-1 (P), middle one to
@@ -166,9 +243,9 @@ struct TmaStep {
                                                      V (&Cc)[C::NA], V (&N)[C::NA]) {
         const V two = V::bc(T(2)), eight = V::bc(T(8));
         V El[3], Wl[3], Ol[3], Em[3], Wm[3], Om[3], Eh[3], Wh[3], Oh[3];
-        brackets<-1, false>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
-        brackets<1, false>(s, r, Eh, Wh, Oh);    // sources at y-1 (cy = +1)
-        brackets<0, false>(s, r, Em, Wm, Om);
+        brackets_any<-1, false>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
+        brackets_any<1, false>(s, r, Eh, Wh, Oh);    // sources at y-1 (cy = +1)
+        brackets_any<0, false>(s, r, Em, Wm, Om);
         // cz = 0: separable (1,2,1) passes over E, then the extra centre weight
         const XRow<V> xl = xpass<V>(El[0], El[1], El[2], two), xm = xpass<V>(Em[0], Em[1], Em[2], two),
                       xh = xpass<V>(Eh[0], Eh[1], Eh[2], two);
