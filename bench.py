@@ -145,7 +145,7 @@ def time_oracle(a, seconds_target=15.0):
     t0 = time.perf_counter()
     fn(m, nsteps=1, **kw)
     t1 = time.perf_counter() - t0
-    steps = int(max(1, min(50, seconds_target / max(t1, 1e-3))))
+    steps = int(max(1, min(1000, seconds_target / max(t1, 1e-3))))
     t0 = time.perf_counter()
     fn(m, nsteps=steps, **kw)
     dt = time.perf_counter() - t0
