@@ -59,8 +59,9 @@ int state_fields(const lbwp_params* p) {
 
 
 bool tma_eligible(const lbwp_params* p) {
-    if (p->scheme == LBWP_MOMENTS && p->ncomp == 2 && p->lattice == 27)
-        return p->dtype == LBWP_F32 ? lbwp::Tma2Plan<float>::eligible(p->nx, p->ny) : lbwp::Tma2Plan<double>::eligible(p->nx, p->ny);
+    if (p->scheme == LBWP_MOMENTS && p->ncomp == 2)
+        return p->dtype == LBWP_F32 ? lbwp::Tma2Plan<float, 27>::eligible(p->nx, p->ny)
+                                    : lbwp::Tma2Plan<double, 27>::eligible(p->nx, p->ny);
     if (!(p->scheme == LBWP_MOMENTS && p->ncomp == 1)) return false;
     return p->dtype == LBWP_F32 ? lbwp::tma_eligible_f32(p->nx, p->ny) : lbwp::tma_eligible_f64(p->nx, p->ny);
 }
@@ -227,16 +228,20 @@ struct TmaCtx final : lbwp_ctx {
 // Two-component TMA variant (lbwp_tma2.cuh): buf[0] = S15 scratch, buf[1] = R, the state (12 of 15 fields used).
 template <typename T>
 struct Tma2Ctx final : lbwp_ctx {
-    lbwp::Tma2Plan<T> plan;
+    lbwp::Tma2PlanBase* planp = nullptr;
     lbwp::XLayout X;
+    ~Tma2Ctx() override { delete planp; }
 
     int prepare() {
-        int rc = plan.setup(X, buf[0]);
+        planp = P.lattice == 27 ? (lbwp::Tma2PlanBase*)new (std::nothrow) lbwp::Tma2Plan<T, 27>()
+                                : (lbwp::Tma2PlanBase*)new (std::nothrow) lbwp::Tma2Plan<T, 19>();
+        if (!planp) return fail(LBWP_ENOMEM, "no two-component TMA plan");
+        int rc = planp->setup(X, buf[0]);
         if (rc) return fail(rc < 0 ? LBWP_EUNSUPPORTED : LBWP_ECUDA, "two-component TMA plan setup failed (%d)", rc);
         return LBWP_OK;
     }
     int step_once() override {
-        int rc = plan.step((T*)buf[1], (T*)buf[0], 1.0 / P.tau, P.A, P.beta, stream);
+        int rc = planp->step(buf[1], buf[0], 1.0 / P.tau, P.A, P.beta, stream);
         if (rc) return fail(LBWP_ECUDA, "two-component step launch: %s", cudaGetErrorString((cudaError_t)rc));
         ++steps;
         return LBWP_OK;

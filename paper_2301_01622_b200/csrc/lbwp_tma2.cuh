@@ -23,7 +23,7 @@ struct Colour2Params {
     T omega, A, beta;
 };
 
-template <typename T>
+template <typename T, int Q>
 __global__ void __launch_bounds__(256) k_colour_collide(const Colour2Params<T> p) {
     const XLayout& L = p.L;
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
@@ -46,8 +46,8 @@ __global__ void __launch_bounds__(256) k_colour_collide(const Colour2Params<T> p
 #pragma unroll
             for (int cx = -1; cx <= 1; ++cx) {
                 const int n2 = cx * cx + cy * cy + cz * cz;
-                if (n2 == 0) continue;
-                const T w = T(3.0 * lattice_w<27>(n2));
+                if (n2 == 0 || (Q == 19 && n2 == 3)) continue;
+                const T w = T(3.0 * lattice_w<Q>(n2));
                 const T f = phi[row + xs[cx + 1]];
                 if (cx) gx += T(cx) * w * f;
                 if (cy) gy += T(cy) * w * f;
@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(256) k_colour_collide(const Colour2Params<T> p
     n.Syz += Ag * ny * nz;
     const T rA = rhoA * irho;
     const T kappa = p.beta * rA * (rho - rhoA);   // beta rhoA rhoB / rho
-    const T c = T(1.0 / 216.0);
+    const T c = Q == 27 ? T(1.0 / 216.0) : T(1.0 / 36.0);
     T out[15];
     out[0] = c * n.da;
     out[1] = c * n.Jx; out[2] = c * n.Jy; out[3] = c * n.Jz;
@@ -131,13 +131,19 @@ __global__ void __launch_bounds__(256) k_tma2_export(XLayout L, const T* __restr
 }
 
 // ---- host side: one two-component plan per dtype ----------------------------------------------------
-template <typename T> struct Tma2Geom;
-template <> struct Tma2Geom<float> { using C = TmaCfg<float, 2, 64, 8, 3, 27, 2>; };
-template <> struct Tma2Geom<double> { using C = TmaCfg<double, 1, 32, 8, 3, 27, 2>; };
+template <typename T, int Q> struct Tma2Geom;
+template <int Q> struct Tma2Geom<float, Q> { using C = TmaCfg<float, 2, 64, 8, 3, Q, 2>; };
+template <int Q> struct Tma2Geom<double, Q> { using C = TmaCfg<double, 1, 32, 8, 3, Q, 2>; };
 
-template <typename T>
-struct Tma2Plan {
-    using C = typename Tma2Geom<T>::C;
+struct Tma2PlanBase {
+    virtual ~Tma2PlanBase() {}
+    virtual int setup(const XLayout& L_, void* s15) = 0;
+    virtual int step(void* raw, void* s15, double omega, double A, double beta, cudaStream_t stream) const = 0;
+};
+
+template <typename T, int Q>
+struct Tma2Plan final : Tma2PlanBase {
+    using C = typename Tma2Geom<T, Q>::C;
     XLayout L;
     CUtensorMap main_map, row_map;   // over the S15 scratch buffer
     int lz = 0, gz = 0, grid = 0;
@@ -145,7 +151,7 @@ struct Tma2Plan {
     static bool eligible(int nx, int ny) { return nx % C::TX == 0 && ny % C::TY == 0; }
     static auto kernel() { return k_step_tma27<T, C, EPI_SFORM, 1>; }
 
-    int setup(const XLayout& L_, void* s15) {
+    int setup(const XLayout& L_, void* s15) override {
         L = L_;
         int rc = make_state_map<T>(&main_map, s15, L, C::BW, C::TY, C::M);
         if (rc) return rc;
@@ -165,13 +171,13 @@ struct Tma2Plan {
     }
 
     // one time step: collide R -> S15, then stream S15 -> R
-    int step(T* raw, T* s15, double omega, double A, double beta, cudaStream_t stream) const {
+    int step(void* raw, void* s15, double omega, double A, double beta, cudaStream_t stream) const override {
         Colour2Params<T> a;
-        a.L = L; a.raw = raw; a.s15 = s15; a.omega = T(omega); a.A = T(A); a.beta = T(beta);
+        a.L = L; a.raw = (const T*)raw; a.s15 = (T*)s15; a.omega = T(omega); a.A = T(A); a.beta = T(beta);
         const dim3 b(32, 8, 1), g((L.nx + 31) / 32, (L.ny + 7) / 8, L.nz);
-        k_colour_collide<T><<<g, b, 0, stream>>>(a);
+        k_colour_collide<T, Q><<<g, b, 0, stream>>>(a);
         TmaStepParams<T> p;
-        p.L = L; p.dst = raw; p.omega = T(omega); p.lz = lz;
+        p.L = L; p.dst = (T*)raw; p.omega = T(omega); p.lz = lz;
         kernel()<<<grid, C::NT + 32, C::SMEM, stream>>>(main_map, row_map, p);
         return (int)cudaGetLastError();
     }

@@ -248,7 +248,8 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
             P[f] = P[f] + Cc[f];
         }
 #else
-        if constexpr (C::NC == 2) S::consume2c(sm, rs, P, Cc, N);
+        if constexpr (C::NC == 2 && C::Q == 27) S::consume2c(sm, rs, P, Cc, N);
+        else if constexpr (C::NC == 2) S::consume2c19(sm, rs, P, Cc, N);
         else if constexpr (C::Q == 27) S::consume(sm, rs, P, Cc, N);
         else S::consume19(sm, rs, P, Cc, N);
 #endif

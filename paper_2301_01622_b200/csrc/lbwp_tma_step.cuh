@@ -28,7 +28,6 @@ struct TmaCfg {
     static constexpr int M = NC_ == 1 ? 10 : 15;      // fields per node in a stage
     static constexpr int NA = NC_ == 1 ? 10 : 11;     // moment sums per node
     static_assert(Q_ == 27 || Q_ == 19, "lattice");
-    static_assert(NC_ == 1 || Q_ == 27, "the two-component stencil is built for D3Q27");
     static constexpr int OX = 16 / (int)sizeof(T);            // halo column sits at OX-1 and OX+TX
     static constexpr int BW = TX + 2 * OX;                    // box width: 16-byte multiple
     static constexpr int ROW = M * BW;                        // elements per tile row [field][BW]
@@ -279,7 +278,7 @@ struct TmaStep {
     __device__ static __forceinline__ void colour_row(const T* __restrict__ s, const int (&r)[C::NPT][3], const V (&E)[3],
                                                       const V (&W)[3], const V (&O)[3], const V& four, V& ae, V& aw, V& ao) {
         constexpr int J = 1 - CY;
-        const V cc = V::bc(T(1.0 / 216.0));
+        const V cc = V::bc(C::Q == 27 ? T(1.0 / 216.0) : T(1.0 / 36.0));
         const V ra[3] = {ld<10, -1>(s, r, J), ld<10, 0>(s, r, J), ld<10, 1>(s, r, J)};
         V AE[3], AW[3], AO[3];
 #pragma unroll
@@ -346,6 +345,77 @@ struct TmaStep {
         const V r0 = ld<14, 0>(s, r, 1), rac = ld<10, 0>(s, r, 1);
         Cc[0] = Cc[0] + r0;
         Cc[10] = vfma(four, mae, Cc[10]) + vfma(rac, r0, t0);
+        N[10] = (maw + mao) + (tin + tz);
+        P[10] = P[10] + ((maw - mao) + (tin - tz));
+    }
+
+    // The same for D3Q19: total moments as in consume19(); the colour sums use the D3Q19 weights x 36
+    // (in-plane (1,2,1)^2 + 8 on the centre; off-plane a plus), K enters with 2 (axis) and 1/sqrt2 (face diagonal).
+    __device__ static __forceinline__ void colour_products(const T* __restrict__ s, const int (&r)[C::NPT][3], int j,
+                                                           const V (&E)[3], const V (&W)[3], const V (&O)[3], bool sides,
+                                                           V (&AE)[3], V (&AW)[3], V (&AO)[3]) {
+        const V cc = V::bc(T(1.0 / 36.0));
+        const V ra[3] = {ld<10, -1>(s, r, j), ld<10, 0>(s, r, j), ld<10, 1>(s, r, j)};
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const V rac = ra[k] * cc;
+            AE[k] = vfma(ra[k], E[k], rac);
+            if (k == 1 || sides) { AW[k] = vfma(ra[k], W[k], rac); AO[k] = ra[k] * O[k]; }
+        }
+    }
+
+    __device__ static __forceinline__ void consume2c19(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
+                                                       V (&Cc)[C::NA], V (&N)[C::NA]) {
+        const V two = V::bc(T(2)), eight = V::bc(T(8));
+        V El[3], Wl[3], Ol[3], Em[3], Wm[3], Om[3], Eh[3], Wh[3], Oh[3];
+        brackets<-1, false>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
+        brackets<1, false>(s, r, Eh, Wh, Oh);    // sources at y-1 (cy = +1)
+        brackets<0, false>(s, r, Em, Wm, Om);
+        {   // total fluid: identical to consume19()
+            const XRow<V> xl = xpass<V>(El[0], El[1], El[2], two), xm = xpass<V>(Em[0], Em[1], Em[2], two),
+                          xh = xpass<V>(Eh[0], Eh[1], Eh[2], two);
+            Mom6<V> me = ypass<V>(xl, xm, xh, two);
+            me.m00 = vfma(eight, Em[1], me.m00);
+            Cc[0] = Cc[0] + me.m00; Cc[1] = Cc[1] + me.m10; Cc[2] = Cc[2] + me.m01;
+            Cc[4] = Cc[4] + me.m20; Cc[5] = Cc[5] + me.m02; Cc[7] = Cc[7] + me.m11;
+            const V wx = Wm[2] + Wm[0], wy = Wh[1] + Wl[1], ox = Om[2] + Om[0], oy = Oh[1] + Ol[1];
+            const V w00 = vfma(two, Wm[1], wx + wy), o00 = vfma(two, Om[1], ox + oy);
+            const V w10 = Wm[2] - Wm[0], o10 = Om[2] - Om[0];
+            const V w01 = Wh[1] - Wl[1], o01 = Oh[1] - Ol[1];
+            const V p00 = w00 + o00, p10 = w10 + o10, p01 = w01 + o01;
+            N[0] = p00; N[1] = p10; N[2] = p01; N[3] = p00;
+            N[4] = wx + ox; N[5] = wy + oy; N[6] = p00;
+            N[7] = V::bc(T(0)); N[8] = p10; N[9] = p01;
+            const V n00 = w00 - o00, n10 = w10 - o10, n01 = w01 - o01;
+            P[0] = P[0] + n00; P[1] = P[1] + n10; P[2] = P[2] + n01; P[3] = P[3] - n00;
+            P[4] = P[4] + (wx - ox); P[5] = P[5] + (wy - oy); P[6] = P[6] + n00;
+            P[8] = P[8] - n10; P[9] = P[9] - n01;
+        }
+        // colour A, first part: sum_c w_c rA (1 + B_c)
+        V AEl[3], AWl[3], AOl[3], AEm[3], AWm[3], AOm[3], AEh[3], AWh[3], AOh[3];
+        colour_products(s, r, 2, El, Wl, Ol, false, AEl, AWl, AOl);   // cy = -1 is row slot 2
+        colour_products(s, r, 0, Eh, Wh, Oh, false, AEh, AWh, AOh);
+        colour_products(s, r, 1, Em, Wm, Om, true, AEm, AWm, AOm);
+        const V rl = vfma(two, AEl[1], AEl[2] + AEl[0]), rm = vfma(two, AEm[1], AEm[2] + AEm[0]),
+                rh = vfma(two, AEh[1], AEh[2] + AEh[0]);
+        const V mae = vfma(eight, AEm[1], vfma(two, rm, rh + rl));
+        const V maw = vfma(two, AWm[1], (AWm[2] + AWm[0]) + (AWh[1] + AWl[1]));
+        const V mao = vfma(two, AOm[1], (AOm[2] + AOm[0]) + (AOh[1] + AOl[1]));
+        // second part: sum_{c != 0} w_c K.c / |c|; weights x 36 / |c|: 2 (axis), 1/sqrt2 (face diagonal)
+        const V kxa = ld<11, 1>(s, r, 1) - ld<11, -1>(s, r, 1);
+        const V kxb = (ld<11, 1>(s, r, 0) - ld<11, -1>(s, r, 0)) + (ld<11, 1>(s, r, 2) - ld<11, -1>(s, r, 2));
+        const V kya = ld<12, 0>(s, r, 0) - ld<12, 0>(s, r, 2);
+        const V kyb = (ld<12, 1>(s, r, 0) - ld<12, 1>(s, r, 2)) + (ld<12, -1>(s, r, 0) - ld<12, -1>(s, r, 2));
+        const V z0 = ld<13, 0>(s, r, 1);
+        const V z1 = (ld<13, 1>(s, r, 1) + ld<13, -1>(s, r, 1)) + (ld<13, 0>(s, r, 0) + ld<13, 0>(s, r, 2));
+        const V da = kxa + kya, db = kxb + kyb;
+        const V f2 = V::bc(T(0.70710678118654752));
+        const V t0 = vfma(two, da, f2 * db);     // cz = 0: axis and in-plane face diagonals
+        const V tin = f2 * da;                   // cz = +-1: (+-1, 0, cz), (0, +-1, cz)
+        const V tz = vfma(two, z0, f2 * z1);     // cz = +-1: c_z K_z of (0,0,cz) and the four above
+        const V r0 = ld<14, 0>(s, r, 1), rac = ld<10, 0>(s, r, 1);
+        Cc[0] = Cc[0] + r0;
+        Cc[10] = (Cc[10] + mae) + vfma(rac, r0, t0);
         N[10] = (maw + mao) + (tin + tz);
         P[10] = P[10] + ((maw - mao) + (tin - tz));
     }
