@@ -44,7 +44,7 @@ def parse_args():
     ap.add_argument("--lattice", type=int, default=27, choices=[19, 27])
     ap.add_argument("--ncomp", type=int, default=1, choices=[1, 2])
     ap.add_argument("--scheme", default="moments", choices=["moments", "populations"])
-    ap.add_argument("--kernel", default="auto", choices=["auto", "gather", "march", "tma"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "gather", "march", "tma", "tma_split"])
     ap.add_argument("--e2e-steps", type=int, default=2, help="host-buffer steps timed for the e2e key (0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()

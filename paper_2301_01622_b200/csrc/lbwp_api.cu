@@ -16,6 +16,7 @@
 #include "lbwp_pop.cuh"
 #include "lbwp_tma_host.cuh"
 #include "lbwp_tma2.cuh"
+#include "lbwp_tma2f.cuh"
 
 namespace {
 
@@ -43,7 +44,7 @@ bool params_ok(const lbwp_params* p) {
     if (p->dtype != LBWP_F32 && p->dtype != LBWP_F64) return false;
     if (p->ncomp != 1 && p->ncomp != 2) return false;
     if (p->scheme != LBWP_MOMENTS && p->scheme != LBWP_POPULATIONS) return false;
-    if (p->kernel < LBWP_KERNEL_AUTO || p->kernel > LBWP_KERNEL_TMA) return false;
+    if (p->kernel < LBWP_KERNEL_AUTO || p->kernel > LBWP_KERNEL_TMA_SPLIT) return false;
     if (p->nx < 1 || p->ny < 1 || p->nz < 1) return false;
     if ((long long)p->nx * p->ny * p->nz > (1ll << 31)) return false;
     if (!(p->tau > 0.5)) return false;  // also rejects NaN
@@ -66,12 +67,16 @@ bool tma_eligible(const lbwp_params* p) {
     return p->dtype == LBWP_F32 ? lbwp::tma_eligible_f32(p->nx, p->ny) : lbwp::tma_eligible_f64(p->nx, p->ny);
 }
 
+// two-component TMA runs: fused form for D3Q27 unless the split form is asked for; D3Q19 is built split only
+bool tma2_fused(const lbwp_params* p) { return p->ncomp == 2 && p->lattice == 27 && p->kernel != LBWP_KERNEL_TMA_SPLIT; }
+
 // kernel variant a context with these params runs (LBWP_KERNEL_AUTO resolved); 0 if not built
 int choose_variant(const lbwp_params* p) {
     const bool march_ok = p->scheme == LBWP_MOMENTS && p->ncomp == 1 && p->lattice == 27;
     switch (p->kernel) {
         case LBWP_KERNEL_AUTO: return tma_eligible(p) ? LBWP_KERNEL_TMA : march_ok ? LBWP_KERNEL_MARCH : LBWP_KERNEL_GATHER;
         case LBWP_KERNEL_TMA: return tma_eligible(p) ? LBWP_KERNEL_TMA : 0;
+        case LBWP_KERNEL_TMA_SPLIT: return (p->ncomp == 2 && tma_eligible(p)) ? LBWP_KERNEL_TMA : 0;
         case LBWP_KERNEL_MARCH: return march_ok ? LBWP_KERNEL_MARCH : 0;
         default: return LBWP_KERNEL_GATHER;
     }
@@ -261,6 +266,49 @@ struct Tma2Ctx final : lbwp_ctx {
     }
 };
 
+// Fused two-component TMA variant (lbwp_tma2f.cuh): two ping-pong state buffers of 16 fields.  buf[cur] = state of
+// time t; buf[cur^1] = state of time t-1 (t >= 1) or the plain moments (t = 0), which lbwp_moments needs.
+template <typename T>
+struct Tma2fCtx final : lbwp_ctx {
+    lbwp::Tma2fPlan<T> plan;
+    lbwp::XLayout X;
+
+    int prepare() {
+        int rc = plan.setup(X, buf);
+        if (rc) return fail(rc < 0 ? LBWP_EUNSUPPORTED : LBWP_ECUDA, "fused two-component TMA plan setup failed (%d)", rc);
+        return LBWP_OK;
+    }
+    int step_once() override {
+        int rc = plan.stencil(lbwp::EPI_SFORM, cur, buf[cur ^ 1], 1.0 / P.tau, P.beta, stream);
+        if (!rc) rc = plan.normals(buf[cur ^ 1], P.A, stream);
+        if (rc) return fail(LBWP_ECUDA, "fused two-component step launch: %s", cudaGetErrorString((cudaError_t)rc));
+        cur ^= 1;
+        ++steps;
+        return LBWP_OK;
+    }
+    int import_dense(const void* ext) override {
+        const dim3 b(32, 8, 1), g((X.nx + 31) / 32, (X.ny + 7) / 8, X.nz);
+        steps = 0;
+        cur = 0;
+        lbwp::k_tma2f_import<T><<<g, b, 0, stream>>>(X, (const T*)ext, (T*)buf[0], (T*)buf[1], T(1.0 / P.tau), T(P.beta));
+        CU(cudaGetLastError());
+        int rc = plan.normals(buf[0], P.A, stream);
+        if (rc) return fail(LBWP_ECUDA, "gradient pass launch: %s", cudaGetErrorString((cudaError_t)rc));
+        return LBWP_OK;
+    }
+    int export_dense(void* ext) override {
+        if (steps == 0) {
+            const dim3 b(32, 8, 1), g((X.nx + 31) / 32, (X.ny + 7) / 8, X.nz);
+            lbwp::k_tma2f_export_raw<T><<<g, b, 0, stream>>>(X, (const T*)buf[cur ^ 1], (T*)ext);
+            CU(cudaGetLastError());
+            return LBWP_OK;
+        }
+        int rc = plan.stencil(lbwp::EPI_MOMENTS, cur ^ 1, ext, 1.0 / P.tau, P.beta, stream);
+        if (rc) return fail(LBWP_ECUDA, "fused two-component export launch: %s", cudaGetErrorString((cudaError_t)rc));
+        return LBWP_OK;
+    }
+};
+
 size_t dense_bytes(const lbwp_ctx* c) { return (size_t)c->M * c->L.nx * c->L.ny * c->L.nz * c->esize; }
 
 int load_moments(lbwp_ctx* c, const void* moments, int on_device) {
@@ -288,7 +336,7 @@ size_t lbwp_state_bytes(const lbwp_params* p) {
     if (variant == 0) return 0;
     if (variant == LBWP_KERNEL_TMA) {
         const lbwp::XLayout X = lbwp::make_xlayout(p->nx, p->ny, p->nz, elem_bytes(p));
-        return (size_t)(p->ncomp == 2 ? 15 : 10) * (size_t)X.field * (size_t)elem_bytes(p);
+        return (size_t)(p->ncomp == 2 ? (tma2_fused(p) ? 16 : 15) : 10) * (size_t)X.field * (size_t)elem_bytes(p);
     }
     const lbwp::Layout L = lbwp::make_layout(p->nx, p->ny, p->nz, elem_bytes(p));
     return (size_t)state_fields(p) * (size_t)L.field * (size_t)elem_bytes(p);
@@ -318,7 +366,10 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
     lbwp_ctx* c = nullptr;
     if (variant == LBWP_KERNEL_TMA) {
         const lbwp::XLayout X = lbwp::make_xlayout(p->nx, p->ny, p->nz, elem_bytes(p));
-        if (p->ncomp == 2) {
+        if (tma2_fused(p)) {
+            if (p->dtype == LBWP_F32) { auto* t = new (std::nothrow) Tma2fCtx<float>(); if (t) t->X = X; c = t; }
+            else { auto* t = new (std::nothrow) Tma2fCtx<double>(); if (t) t->X = X; c = t; }
+        } else if (p->ncomp == 2) {
             if (p->dtype == LBWP_F32) { auto* t = new (std::nothrow) Tma2Ctx<float>(); if (t) t->X = X; c = t; }
             else { auto* t = new (std::nothrow) Tma2Ctx<double>(); if (t) t->X = X; c = t; }
         } else if (p->dtype == LBWP_F32) { auto* t = new (std::nothrow) TmaCtx<float>(); if (t) t->X = X; c = t; }
@@ -359,7 +410,10 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
     }
     c->variant = variant;
     if (variant == LBWP_KERNEL_TMA) {
-        if (p->ncomp == 2) {
+        if (tma2_fused(p)) {
+            rc = p->dtype == LBWP_F32 ? static_cast<Tma2fCtx<float>*>(c)->prepare() : static_cast<Tma2fCtx<double>*>(c)->prepare();
+            c->launches_per_step = 2;
+        } else if (p->ncomp == 2) {
             rc = p->dtype == LBWP_F32 ? static_cast<Tma2Ctx<float>*>(c)->prepare() : static_cast<Tma2Ctx<double>*>(c)->prepare();
             c->launches_per_step = 2;
         } else {
@@ -369,7 +423,8 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
     }
     snprintf(c->name, sizeof(c->name), "%s%d_%s%s",
              p->scheme == LBWP_POPULATIONS ? "pop_pull" : (variant == LBWP_KERNEL_TMA ? "tma" : variant == LBWP_KERNEL_MARCH ? "march" : "gather"),
-             p->lattice, p->dtype == LBWP_F32 ? "f32" : "f64", p->ncomp == 2 ? "_c2" : "");
+             p->lattice, p->dtype == LBWP_F32 ? "f32" : "f64",
+             p->ncomp != 2 ? "" : (variant == LBWP_KERNEL_TMA && !tma2_fused(p)) ? "_c2split" : "_c2");
     rc = load_moments(c, moments, moments_on_device);
     if (rc) return bail(rc);
     *out = c;

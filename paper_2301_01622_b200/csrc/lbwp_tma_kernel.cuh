@@ -124,6 +124,64 @@ __device__ __forceinline__ void store_raw2_node(const XLayout& L, T* __restrict_
     d[11 * F] = (a[10] + a[10] - rho) * rcp_t<T>(rho);
 }
 
+// Fused two-component mode (C::NC == 3): finished sums (drho, j, dP_aa, P_ab, rhoA) -> the twelve state fields
+// S-form after BGK (Eq. 8, no perturbation yet), rA = rhoA/rho, kappa = beta rhoA rhoB/rho (x 1/216); the
+// interface fields 12..15 are written by the gradient pass (lbwp_tma2f.cuh).
+template <typename T>
+__device__ __forceinline__ void store_state2f(const XLayout& L, T* __restrict__ dst, const T (&a)[11], T omega, T beta, int x,
+                                              int y, int z) {
+    const T c = T(1.0 / 216.0);
+    const T rho = T(1) + a[0];
+    const T irho = rcp_t<T>(rho);
+    const T ux = a[1] * irho, uy = a[2] * irho, uz = a[3] * irho;
+    const T om1 = T(1) - omega;
+    const T wx = omega * a[1], wy = omega * a[2], wz = omega * a[3];
+    const T iso = a[0] * T(1.0 / 3.0);
+    const T sxx = fma(wx, ux, om1 * (a[4] - iso));
+    const T syy = fma(wy, uy, om1 * (a[5] - iso));
+    const T szz = fma(wz, uz, om1 * (a[6] - iso));
+    const T sxy = fma(wx, uy, om1 * a[7]);
+    const T sxz = fma(wx, uz, om1 * a[8]);
+    const T syz = fma(wy, uz, om1 * a[9]);
+    T out[12];
+    out[0] = c * fma(T(-1.5), sxx + syy + szz, a[0]);
+    out[1] = (T(3) * c) * a[1];
+    out[2] = (T(3) * c) * a[2];
+    out[3] = (T(3) * c) * a[3];
+    out[4] = (T(4.5) * c) * sxx;
+    out[5] = (T(4.5) * c) * syy;
+    out[6] = (T(4.5) * c) * szz;
+    out[7] = (T(9) * c) * sxy;
+    out[8] = (T(9) * c) * sxz;
+    out[9] = (T(9) * c) * syz;
+    const T rA = a[10] * irho;
+    out[10] = rA;
+    out[11] = (c * beta) * (rA * (rho - a[10]));   // beta rhoA rhoB / rho
+    const long long F = L.field;
+    T* __restrict__ d = dst + xidx(L, x, y, z);
+#pragma unroll
+    for (int f = 0; f < 12; ++f) d[f * F] = out[f];
+    if (x == 0 || x == L.nx - 1) {
+        T* __restrict__ g = x == 0 ? d + L.nx : d - L.nx;
+#pragma unroll
+        for (int f = 0; f < 12; ++f) g[f * F] = out[f];
+    }
+}
+
+// ... and the same sums written as the external moments (rhoA, rhoB, u, P), dense [11][nz][ny][nx]
+template <typename T>
+__device__ __forceinline__ void store_dense2(const XLayout& L, T* __restrict__ ext, const T (&a)[11], int x, int y, int z) {
+    const long long n = (long long)L.nx * L.ny * L.nz;
+    T* __restrict__ d = ext + ((long long)z * L.ny + y) * L.nx + x;
+    const T rho = T(1) + a[0];
+    const T irho = rcp_t<T>(rho);
+    d[0] = a[10];
+    d[n] = rho - a[10];
+    d[2 * n] = a[1] * irho; d[3 * n] = a[2] * irho; d[4 * n] = a[3] * irho;
+    d[5 * n] = a[4] + T(1.0 / 3.0); d[6 * n] = a[5] + T(1.0 / 3.0); d[7 * n] = a[6] + T(1.0 / 3.0);
+    d[8 * n] = a[7]; d[9 * n] = a[8]; d[10 * n] = a[9];
+}
+
 // Work decomposition: item = (z chunk, tile row, tile column), x fastest, so that items handled at
 // the same time by neighbouring CTAs are spatial neighbours and their halo reads meet in L2.
 struct TmaItem {
@@ -248,7 +306,8 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
             P[f] = P[f] + Cc[f];
         }
 #else
-        if constexpr (C::NC == 2 && C::Q == 27) S::consume2c(sm, rs, P, Cc, N);
+        if constexpr (C::NC == 3) S::consume2f(sm, rs, P, Cc, N);
+        else if constexpr (C::NC == 2 && C::Q == 27) S::consume2c(sm, rs, P, Cc, N);
         else if constexpr (C::NC == 2) S::consume2c19(sm, rs, P, Cc, N);
         else if constexpr (C::Q == 27) S::consume(sm, rs, P, Cc, N);
         else S::consume19(sm, rs, P, Cc, N);
@@ -259,7 +318,18 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
             // collision over the thread's nodes at once, except where it costs registers the stencil needs
             // (fp32 D3Q27 at 96 registers: packed epilogue spills and measured 56 vs 62 GLUPS)
             constexpr bool kVectorEpilogue = C::PX || !(C::Q == 27 && C::NPT == 2);
-            if constexpr (C::NC == 2) {
+            if constexpr (C::NC == 3) {
+#pragma unroll
+                for (int n = 0; n < C::NPT; ++n) {
+                    T acc[C::NA];
+#pragma unroll
+                    for (int f = 0; f < C::NA; ++f) acc[f] = P[f].get(n);
+                    if (EPI == EPI_SFORM)
+                        store_state2f<T>(L, p.dst, acc, p.omega, p.beta, ct.x0 + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
+                    else
+                        store_dense2<T>(L, p.dst, acc, ct.x0 + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
+                }
+            } else if constexpr (C::NC == 2) {
 #pragma unroll
                 for (int n = 0; n < C::NPT; ++n) {
                     T acc[C::NA];

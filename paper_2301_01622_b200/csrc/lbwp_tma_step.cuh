@@ -12,6 +12,7 @@ struct TmaStepParams {
     T* __restrict__ dst;   // EPI_SFORM: XLayout fields; EPI_MOMENTS: dense external [10][nz][ny][nx]
     T omega;               // 1/tau (reading C3)
     int lz;                // z planes per chunk
+    T beta = T(0);         // recolouring strength (fused two-component mode only)
 };
 
 // Compile-time geometry of one instance.
@@ -25,8 +26,10 @@ template <typename T, int NPT_, int TX_, int TY_, int NS_, int Q_ = 27, int NC_ 
 struct TmaCfg {
     static constexpr int NPT = NPT_, TX = TX_, TY = TY_, NS = NS_, Q = Q_, NC = NC_, PX = PX_;
     static_assert(PX_ == 0 || (NPT_ == 2 && sizeof(T) == 4 && NC_ == 1), "x-paired mode: fp32, two nodes, one component");
-    static constexpr int M = NC_ == 1 ? 10 : 15;      // fields per node in a stage
-    static constexpr int NA = NC_ == 1 ? 10 : 11;     // moment sums per node
+    // NC = 3: fused two-component mode (lbwp_tma2f.cuh): sixteen fields in (unperturbed S-form, rA, kappa, and
+    // the interface fields (A/2)|G|, n of the gradient pass), perturbation and recolouring applied per direction.
+    static constexpr int M = NC_ == 1 ? 10 : NC_ == 2 ? 15 : 16;   // fields per node in a stage
+    static constexpr int NA = NC_ == 1 ? 10 : 11;                   // moment sums per node
     static_assert(Q_ == 27 || Q_ == 19, "lattice");
     static constexpr int OX = 16 / (int)sizeof(T);            // halo column sits at OX-1 and OX+TX
     static constexpr int BW = TX + 2 * OX;                    // box width: 16-byte multiple
@@ -416,6 +419,121 @@ struct TmaStep {
         const V r0 = ld<14, 0>(s, r, 1), rac = ld<10, 0>(s, r, 1);
         Cc[0] = Cc[0] + r0;
         Cc[10] = (Cc[10] + mae) + vfma(rac, r0, t0);
+        N[10] = (maw + mao) + (tin + tz);
+        P[10] = P[10] + ((maw - mao) + (tin - tz));
+    }
+
+    // ---- fused two-component mode (C::NC == 3, D3Q27) ----
+    // Fields: 0..9 S-form of the total fluid after BGK only (x 1/216), 10 rA = rhoA/rho, 11 kappa = beta rhoA rhoB/rho
+    // (x 1/216), 12 gh = (A/2)|G| (x 1/216), 13..15 n = G/|G| (0 where |G| vanishes, reading C8).
+    // Perturbation (reading C6): every direction's bracket gains gh ((c.n)^2 - 1); with e = cx nx + cy ny this is
+    //   E += gh (e^2 - 1),   W += gh (e^2 - 1) + gh nz^2,   O += 2 gh e nz      (bracket = E + cz^2 Szz + cz O),
+    // and the rest direction also gains the population (A/3)|G| = 144 gh.  Recolouring as in consume2c, K = kappa n.
+    template <int CY>
+    __device__ static __forceinline__ void colour_fold(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&E)[3], V (&W)[3],
+                                                       V (&O)[3], V (&ra)[3], V (&kx)[3], V (&ky)[3], V (&kz)[3], V& gh_mid) {
+        constexpr int J = 1 - CY;
+        const V zero = V::bc(T(0));
+#pragma unroll
+        for (int cx = -1; cx <= 1; ++cx) {
+            const int k = cx + 1;
+            V gh, nx, ny, nz, kc;
+            if (cx == -1) { ra[k] = ld<10, -1>(s, r, J); kc = ld<11, -1>(s, r, J); gh = ld<12, -1>(s, r, J);
+                            nx = ld<13, -1>(s, r, J); ny = ld<14, -1>(s, r, J); nz = ld<15, -1>(s, r, J); }
+            if (cx == 0) { ra[k] = ld<10, 0>(s, r, J); kc = ld<11, 0>(s, r, J); gh = ld<12, 0>(s, r, J);
+                           nx = ld<13, 0>(s, r, J); ny = ld<14, 0>(s, r, J); nz = ld<15, 0>(s, r, J); }
+            if (cx == 1) { ra[k] = ld<10, 1>(s, r, J); kc = ld<11, 1>(s, r, J); gh = ld<12, 1>(s, r, J);
+                           nx = ld<13, 1>(s, r, J); ny = ld<14, 1>(s, r, J); nz = ld<15, 1>(s, r, J); }
+            kx[k] = kc * nx; ky[k] = kc * ny; kz[k] = kc * nz;
+            const V gz = gh * nz;
+            const V Eg = E[k] - gh, Wg = W[k] - gh;
+            if (cx == 0 && CY == 0) {
+                E[k] = Eg;
+                W[k] = vfma(gz, nz, Wg);
+                gh_mid = gh;
+            } else {
+                V e;
+                if (cx == 0) e = CY > 0 ? ny : zero - ny;
+                else if (CY == 0) e = cx > 0 ? nx : zero - nx;
+                else if (cx > 0) e = CY > 0 ? nx + ny : nx - ny;
+                else e = CY > 0 ? ny - nx : (zero - nx) - ny;
+                const V t = gh * e;
+                E[k] = vfma(t, e, Eg);
+                W[k] = vfma(gz, nz, vfma(t, e, Wg));
+                O[k] = vfma(t + t, nz, O[k]);
+            }
+        }
+    }
+
+    __device__ static __forceinline__ void consume2f(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
+                                                     V (&Cc)[C::NA], V (&N)[C::NA]) {
+        const V four = V::bc(T(4));
+        const V cc = V::bc(T(1.0 / 216.0));
+        V El[3], Wl[3], Ol[3], Em[3], Wm[3], Om[3], Eh[3], Wh[3], Oh[3];
+        V ral[3], ram[3], rah[3], kxl[3], kxm[3], kxh[3], kyl[3], kym[3], kyh[3], kzl[3], kzm[3], kzh[3], ghc, ghu;
+        brackets<-1, true>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
+        colour_fold<-1>(s, r, El, Wl, Ol, ral, kxl, kyl, kzl, ghu);
+        brackets<1, true>(s, r, Eh, Wh, Oh);    // sources at y-1 (cy = +1)
+        colour_fold<1>(s, r, Eh, Wh, Oh, rah, kxh, kyh, kzh, ghu);
+        brackets<0, true>(s, r, Em, Wm, Om);
+        colour_fold<0>(s, r, Em, Wm, Om, ram, kxm, kym, kzm, ghc);
+        {   // total fluid: identical to consume()
+            const Mom6<V> me = ypass<V>(xpass<V>(El[0], El[1], El[2], four), xpass<V>(Em[0], Em[1], Em[2], four),
+                                        xpass<V>(Eh[0], Eh[1], Eh[2], four), four);
+            const Mom6<V> mw = ypass<V>(xpass<V>(Wl[0], Wl[1], Wl[2], four), xpass<V>(Wm[0], Wm[1], Wm[2], four),
+                                        xpass<V>(Wh[0], Wh[1], Wh[2], four), four);
+            const Mom6<V> mo = ypass<V>(xpass<V>(Ol[0], Ol[1], Ol[2], four), xpass<V>(Om[0], Om[1], Om[2], four),
+                                        xpass<V>(Oh[0], Oh[1], Oh[2], four), four);
+            Cc[0] = vfma(four, me.m00, Cc[0]);
+            Cc[1] = vfma(four, me.m10, Cc[1]);
+            Cc[2] = vfma(four, me.m01, Cc[2]);
+            Cc[4] = vfma(four, me.m20, Cc[4]);
+            Cc[5] = vfma(four, me.m02, Cc[5]);
+            Cc[7] = vfma(four, me.m11, Cc[7]);
+            const V p00 = mw.m00 + mo.m00, p10 = mw.m10 + mo.m10, p01 = mw.m01 + mo.m01;
+            N[0] = p00; N[1] = p10; N[2] = p01; N[3] = p00;
+            N[4] = mw.m20 + mo.m20; N[5] = mw.m02 + mo.m02; N[6] = p00;
+            N[7] = mw.m11 + mo.m11; N[8] = p10; N[9] = p01;
+            const V n00 = mw.m00 - mo.m00, n10 = mw.m10 - mo.m10, n01 = mw.m01 - mo.m01;
+            P[0] = P[0] + n00; P[1] = P[1] + n10; P[2] = P[2] + n01; P[3] = P[3] - n00;
+            P[4] = P[4] + (mw.m20 - mo.m20); P[5] = P[5] + (mw.m02 - mo.m02); P[6] = P[6] + n00;
+            P[7] = P[7] + (mw.m11 - mo.m11); P[8] = P[8] - n10; P[9] = P[9] - n01;
+        }
+        // colour A, first part: sum_c w_c rA (1 + B_c) with the perturbed brackets; zeroth in-plane moment only
+        auto a_row = [&](const V (&ra)[3], const V (&E)[3], const V (&W)[3], const V (&O)[3], V& ae, V& aw, V& ao) {
+            V AE[3], AW[3], AO[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const V rac = ra[k] * cc;
+                AE[k] = vfma(ra[k], E[k], rac);
+                AW[k] = vfma(ra[k], W[k], rac);
+                AO[k] = ra[k] * O[k];
+            }
+            ae = vfma(four, AE[1], AE[2] + AE[0]);
+            aw = vfma(four, AW[1], AW[2] + AW[0]);
+            ao = vfma(four, AO[1], AO[2] + AO[0]);
+        };
+        V ael, awl, aol, aem, awm, aom, aeh, awh, aoh;
+        a_row(ral, El, Wl, Ol, ael, awl, aol);
+        a_row(rah, Eh, Wh, Oh, aeh, awh, aoh);
+        a_row(ram, Em, Wm, Om, aem, awm, aom);
+        const V mae = vfma(four, aem, aeh + ael), maw = vfma(four, awm, awh + awl), mao = vfma(four, aom, aoh + aol);
+        // second part: sum_{c != 0} w_c K.c / |c|; weights x 216 / |c|: 16 (axis), 4/sqrt2 (face), 1/sqrt3 (corner)
+        const V kxa = kxm[2] - kxm[0];
+        const V kxb = (kxh[2] - kxh[0]) + (kxl[2] - kxl[0]);
+        const V kya = kyh[1] - kyl[1];
+        const V kyb = (kyh[2] - kyl[2]) + (kyh[0] - kyl[0]);
+        const V z0 = kzm[1];
+        const V z1 = (kzm[2] + kzm[0]) + (kzh[1] + kzl[1]);
+        const V z2 = (kzh[2] + kzh[0]) + (kzl[2] + kzl[0]);
+        const V da = kxa + kya, db = kxb + kyb;
+        const V f1 = V::bc(T(16)), f2 = V::bc(T(2.8284271247461903)), f3 = V::bc(T(0.57735026918962576));
+        const V t0 = vfma(f1, da, f2 * db);
+        const V tin = vfma(f2, da, f3 * db);
+        const V tz = vfma(f1, z0, vfma(f2, z1, f3 * z2));
+        const V r0 = V::bc(T(144)) * ghc;   // (A/3)|G| in population units
+        Cc[0] = Cc[0] + r0;
+        Cc[10] = vfma(four, mae, Cc[10]) + vfma(ram[1], r0, t0);
         N[10] = (maw + mao) + (tin + tz);
         P[10] = P[10] + ((maw - mao) + (tin - tz));
     }

@@ -18,7 +18,7 @@ LIB_PATH = os.environ.get("LBWP_LIB") or os.path.join(_PKG, "liblbwp.so")   # LB
 
 LBWP_F32, LBWP_F64 = 0, 1
 LBWP_MOMENTS, LBWP_POPULATIONS = 0, 1
-KERNELS = {"auto": 0, "gather": 1, "march": 2, "tma": 3}
+KERNELS = {"auto": 0, "gather": 1, "march": 2, "tma": 3, "tma_split": 4}
 EXPORTS = ["lbwp_state_bytes", "lbwp_num_moments", "lbwp_init", "lbwp_step", "lbwp_moments",
            "lbwp_set_moments", "lbwp_steps_done", "lbwp_launches_per_step", "lbwp_kernel_name",
            "lbwp_sync", "lbwp_destroy", "lbwp_last_error"]

@@ -183,8 +183,8 @@ def test_config3_scaled_droplets(lbwp, oracle, dtype, lattice):
 @pytest.mark.parametrize("dtype,shape", [("f32", (64, 24, 20)), ("f32", (128, 16, 37)), ("f32", (64, 8, 2)),
                                          ("f64", (32, 24, 20)), ("f64", (64, 16, 5))])
 @pytest.mark.parametrize("steps,tau", [(1, 1.0), (30, 0.7)])
-@pytest.mark.parametrize("lattice", [27, 19])
-def test_tma_two_component(lbwp, oracle, dtype, shape, steps, tau, lattice):
+@pytest.mark.parametrize("lattice,kernel", [(27, "tma"), (27, "tma_split"), (19, "tma")])
+def test_tma_two_component(lbwp, oracle, dtype, shape, steps, tau, lattice, kernel):
     nx, ny, nz = shape
     tg = wl.taylor_green(0, shape=shape)
     m = wl.droplets(0, [(0.3 * nx, 0.5 * ny, 0.5 * nz), (0.95 * nx, 0.1 * ny, 0.6 * nz)], 0.3 * min(ny, nx),
@@ -192,11 +192,13 @@ def test_tma_two_component(lbwp, oracle, dtype, shape, steps, tau, lattice):
     cfg = dict(name="tma2_q%d_%s_%s" % (lattice, dtype, "x".join(map(str, shape))), moments=m, lattice=lattice, ncomp=2,
                tau=tau, A=0.01, beta=0.7, dtype=dtype)
     m0 = wl.as_dtype(m, dtype)
-    with lbwp.Lbwp(m0, lattice=lattice, dtype=dtype, ncomp=2, tau=tau, A=0.01, beta=0.7, kernel="tma") as sim:
-        assert sim.kernel_name == "tma%d_%s_c2" % (lattice, dtype) and sim.launches_per_step == 2
+    split = kernel == "tma_split" or lattice == 19
+    with lbwp.Lbwp(m0, lattice=lattice, dtype=dtype, ncomp=2, tau=tau, A=0.01, beta=0.7, kernel=kernel) as sim:
+        assert sim.kernel_name == "tma%d_%s_c2%s" % (lattice, dtype, "split" if split else "")
+        assert sim.launches_per_step == 2
         back = sim.moments_host()          # t = 0: the input, up to the j = rho u round trip
         assert np.abs(back.astype(np.float64) - m0).max() <= (3e-7 if dtype == "f32" else 1e-15)
-    got, ref = check(lbwp, oracle, cfg, steps, kernel="tma")
+    got, ref = check(lbwp, oracle, cfg, steps, kernel=kernel)
     agree = np.mean(np.sign(got[0].astype(np.float64) - got[1]) == np.sign(ref[0] - ref[1]))
     assert agree >= 0.9999
 
