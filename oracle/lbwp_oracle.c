@@ -17,9 +17,10 @@
  *       independent numpy regularised-BGK-with-populations, dense brute force)
  *   two-component colour-gradient .. the operator formulas are not printed in
  *       the paper (PAPER.md:91 defers to ref. [25]); reading C6 is pinned only
- *       internally (A=0 reduction, colour mass conservation, zero mass/momentum
- *       of the perturbation, Laplace law).  Against the paper's own code and
- *       figures: PARITY UNPINNED.
+ *       by what the mathematics fixes (A=0 reduction, colour mass and momentum
+ *       conservation, uniform mixture, interface width, Laplace law with
+ *       sigma = (2/9) A tau).  Against the paper's own code and figures:
+ *       PARITY UNPINNED.
  *   population-storing BGK (comparison kernel's mini-oracle): pinned by
  *       conservation + Taylor-Green viscosity only.
  *
