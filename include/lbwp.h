@@ -52,11 +52,12 @@ enum lbwp_kernel {
     LBWP_KERNEL_AUTO = 0,   /* fastest kernel built for the combination */
     LBWP_KERNEL_GATHER = 1, /* one thread per node, 27/19-neighbour gather through L1/L2 */
     LBWP_KERNEL_MARCH = 2,  /* shared-memory tiles, z-marching register accumulators (any box size) */
-    LBWP_KERNEL_TMA_SPLIT = 4, /* two-component only: collide pass + TMA stencil pass (the paper's split form); what
-                               LBWP_KERNEL_TMA uses for two-component D3Q19 */
+    LBWP_KERNEL_TMA_SPLIT = 4, /* two-component only: collide pass + TMA stencil pass (the paper's split form),
+                               kept for comparison with the fused form LBWP_KERNEL_TMA uses */
     LBWP_KERNEL_TMA = 3     /* TMA-fed stencil on the collided ("S-form") moments, collision as epilogue:
                                D3Q27 and D3Q19, nx a multiple of 64 (fp32) / 32 (fp64), ny of 8; two-component runs
-                               take two launches per step (collide pass, then the stencil) */
+                               take two launches per step (the stencil with the colour operators, then the
+                               phase-field gradient) */
 };
 
 typedef struct lbwp_params {

@@ -67,8 +67,8 @@ bool tma_eligible(const lbwp_params* p) {
     return p->dtype == LBWP_F32 ? lbwp::tma_eligible_f32(p->nx, p->ny) : lbwp::tma_eligible_f64(p->nx, p->ny);
 }
 
-// two-component TMA runs: fused form for D3Q27 unless the split form is asked for; D3Q19 is built split only
-bool tma2_fused(const lbwp_params* p) { return p->ncomp == 2 && p->lattice == 27 && p->kernel != LBWP_KERNEL_TMA_SPLIT; }
+// two-component TMA runs: fused form unless the split form is asked for
+bool tma2_fused(const lbwp_params* p) { return p->ncomp == 2 && p->kernel != LBWP_KERNEL_TMA_SPLIT; }
 
 // kernel variant a context with these params runs (LBWP_KERNEL_AUTO resolved); 0 if not built
 int choose_variant(const lbwp_params* p) {
@@ -270,29 +270,32 @@ struct Tma2Ctx final : lbwp_ctx {
 // time t; buf[cur^1] = state of time t-1 (t >= 1) or the plain moments (t = 0), which lbwp_moments needs.
 template <typename T>
 struct Tma2fCtx final : lbwp_ctx {
-    lbwp::Tma2fPlan<T> plan;
+    lbwp::Tma2fPlanBase* planp = nullptr;
     lbwp::XLayout X;
+    ~Tma2fCtx() override { delete planp; }
 
     int prepare() {
-        int rc = plan.setup(X, buf);
+        planp = P.lattice == 27 ? (lbwp::Tma2fPlanBase*)new (std::nothrow) lbwp::Tma2fPlan<T, 27>()
+                                : (lbwp::Tma2fPlanBase*)new (std::nothrow) lbwp::Tma2fPlan<T, 19>();
+        if (!planp) return fail(LBWP_ENOMEM, "no fused two-component TMA plan");
+        int rc = planp->setup(X, buf);
         if (rc) return fail(rc < 0 ? LBWP_EUNSUPPORTED : LBWP_ECUDA, "fused two-component TMA plan setup failed (%d)", rc);
         return LBWP_OK;
     }
     int step_once() override {
-        int rc = plan.stencil(lbwp::EPI_SFORM, cur, buf[cur ^ 1], 1.0 / P.tau, P.beta, stream);
-        if (!rc) rc = plan.normals(buf[cur ^ 1], P.A, stream);
+        int rc = planp->stencil(lbwp::EPI_SFORM, cur, buf[cur ^ 1], 1.0 / P.tau, P.beta, stream);
+        if (!rc) rc = planp->normals(buf[cur ^ 1], P.A, stream);
         if (rc) return fail(LBWP_ECUDA, "fused two-component step launch: %s", cudaGetErrorString((cudaError_t)rc));
         cur ^= 1;
         ++steps;
         return LBWP_OK;
     }
     int import_dense(const void* ext) override {
-        const dim3 b(32, 8, 1), g((X.nx + 31) / 32, (X.ny + 7) / 8, X.nz);
         steps = 0;
         cur = 0;
-        lbwp::k_tma2f_import<T><<<g, b, 0, stream>>>(X, (const T*)ext, (T*)buf[0], (T*)buf[1], T(1.0 / P.tau), T(P.beta));
-        CU(cudaGetLastError());
-        int rc = plan.normals(buf[0], P.A, stream);
+        int rc = planp->import_state(ext, buf[0], buf[1], 1.0 / P.tau, P.beta, stream);
+        if (rc) return fail(LBWP_ECUDA, "import launch: %s", cudaGetErrorString((cudaError_t)rc));
+        rc = planp->normals(buf[0], P.A, stream);
         if (rc) return fail(LBWP_ECUDA, "gradient pass launch: %s", cudaGetErrorString((cudaError_t)rc));
         return LBWP_OK;
     }
@@ -303,7 +306,7 @@ struct Tma2fCtx final : lbwp_ctx {
             CU(cudaGetLastError());
             return LBWP_OK;
         }
-        int rc = plan.stencil(lbwp::EPI_MOMENTS, cur ^ 1, ext, 1.0 / P.tau, P.beta, stream);
+        int rc = planp->stencil(lbwp::EPI_MOMENTS, cur ^ 1, ext, 1.0 / P.tau, P.beta, stream);
         if (rc) return fail(LBWP_ECUDA, "fused two-component export launch: %s", cudaGetErrorString((cudaError_t)rc));
         return LBWP_OK;
     }

@@ -1,4 +1,4 @@
-// lbwp_tma2f.cuh -- two-component colour-gradient runs (reading C6), fused form (D3Q27).
+// lbwp_tma2f.cuh -- two-component colour-gradient runs (reading C6), fused form (D3Q27 and D3Q19).
 //
 // State (two ping-pong buffers, XLayout, 16 fields each):
 //   0..9   S-form of the total fluid after BGK only (x 1/216)      } written by the stencil kernel's epilogue
@@ -27,7 +27,7 @@ struct Normal2Params {
 };
 
 // One thread per (x, y) column and ZC consecutive planes; the ZC + 2 planes of 3 x 3 rA values it needs sit in registers.
-template <typename T, int ZC>
+template <typename T, int Q, int ZC>
 __global__ void __launch_bounds__(256) k_colour_normal(const Normal2Params<T> p) {
     const XLayout& L = p.L;
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
@@ -72,8 +72,9 @@ __global__ void __launch_bounds__(256) k_colour_normal(const Normal2Params<T> p)
 #pragma unroll
                 for (int cx = -1; cx <= 1; ++cx) {
                     const int n2 = cx * cx + cy * cy + cz * cz;
-                    if (n2 == 0) continue;
-                    const T w = T(6.0 * (n2 == 1 ? 2.0 / 27.0 : n2 == 2 ? 1.0 / 54.0 : 1.0 / 216.0));
+                    if (n2 == 0 || (Q == 19 && n2 == 3)) continue;
+                    const T w = Q == 27 ? T(6.0 * (n2 == 1 ? 2.0 / 27.0 : n2 == 2 ? 1.0 / 54.0 : 1.0 / 216.0))
+                                        : T(6.0 * (n2 == 1 ? 1.0 / 18.0 : 1.0 / 36.0));
                     const T f = cz < 0 ? lo[cy + 1][cx + 1] : cz == 0 ? mid[cy + 1][cx + 1] : hi[cy + 1][cx + 1];
                     if (cx) gx += T(cx) * w * f;
                     if (cy) gy += T(cy) * w * f;
@@ -83,7 +84,7 @@ __global__ void __launch_bounds__(256) k_colour_normal(const Normal2Params<T> p)
         const T ig = g2 > T(1e-10) ? T(1) / sqrt(g2) : T(0);   // reading C8
         const T g = g2 * ig;
         T out[4];
-        out[0] = T(1.0 / 216.0) * T(0.5) * p.A * g;
+        out[0] = (Q == 27 ? T(1.0 / 216.0) : T(1.0 / 36.0)) * T(0.5) * p.A * g;
         out[1] = gx * ig; out[2] = gy * ig; out[3] = gz * ig;
         T* __restrict__ d = p.state + 12 * F + (long long)z * L.plane + off[1][1];
 #pragma unroll
@@ -97,7 +98,7 @@ __global__ void __launch_bounds__(256) k_colour_normal(const Normal2Params<T> p)
 }
 
 // dense external moments [11][nz][ny][nx] (rhoA, rhoB, u, P) -> state fields 0..11 (and a plain copy for t = 0)
-template <typename T>
+template <typename T, int Q>
 __global__ void __launch_bounds__(256) k_tma2f_import(XLayout L, const T* __restrict__ ext, T* __restrict__ state,
                                                       T* __restrict__ raw, T omega, T beta) {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
@@ -117,7 +118,7 @@ __global__ void __launch_bounds__(256) k_tma2f_import(XLayout L, const T* __rest
     for (int k = 0; k < 3; ++k) a[4 + k] = T((double)m[5 + k] - 1.0 / 3.0);
     for (int k = 0; k < 3; ++k) a[7 + k] = m[8 + k];
     a[10] = m[0];
-    store_state2f<T>(L, state, a, omega, beta, x, y, z);
+    store_state2f<T, Q>(L, state, a, omega, beta, x, y, z);
 }
 
 template <typename T>
@@ -134,13 +135,21 @@ __global__ void __launch_bounds__(256) k_tma2f_export_raw(XLayout L, const T* __
 }
 
 // ---- host side ---------------------------------------------------------------------------------------
-template <typename T> struct Tma2fGeom;
-template <> struct Tma2fGeom<float> { using C = TmaCfg<float, 2, 64, 8, 3, 27, 3>; };
-template <> struct Tma2fGeom<double> { using C = TmaCfg<double, 1, 32, 8, 3, 27, 3>; };
+template <typename T, int Q> struct Tma2fGeom;
+template <int Q> struct Tma2fGeom<float, Q> { using C = TmaCfg<float, 2, 64, 8, 3, Q, 3>; };
+template <int Q> struct Tma2fGeom<double, Q> { using C = TmaCfg<double, 1, 32, 8, 3, Q, 3>; };
 
-template <typename T>
-struct Tma2fPlan {
-    using C = typename Tma2fGeom<T>::C;
+struct Tma2fPlanBase {
+    virtual ~Tma2fPlanBase() {}
+    virtual int setup(const XLayout& L_, void* const buf[2]) = 0;
+    virtual int stencil(int epi, int from, void* dst, double omega, double beta, cudaStream_t stream) const = 0;
+    virtual int normals(void* state, double A, cudaStream_t stream) const = 0;
+    virtual int import_state(const void* ext, void* state, void* raw, double omega, double beta, cudaStream_t stream) const = 0;
+};
+
+template <typename T, int Q>
+struct Tma2fPlan final : Tma2fPlanBase {
+    using C = typename Tma2fGeom<T, Q>::C;
     XLayout L;
     CUtensorMap main_map[2], row_map[2];
     int lz = 0, gz = 0, grid = 0;
@@ -149,7 +158,7 @@ struct Tma2fPlan {
     template <int EPI>
     static auto kernel() { return k_step_tma27<T, C, EPI, 1>; }
 
-    int setup(const XLayout& L_, void* const buf[2]) {
+    int setup(const XLayout& L_, void* const buf[2]) override {
         L = L_;
         for (int k = 0; k < 2; ++k) {
             int rc = make_state_map<T>(&main_map[k], buf[k], L, C::BW, C::TY, C::M);
@@ -173,7 +182,7 @@ struct Tma2fPlan {
     }
 
     // stencil pass from buffer `from`: EPI_SFORM -> state fields 0..11 of dst, EPI_MOMENTS -> dense moments in dst
-    int stencil(int epi, int from, void* dst, double omega, double beta, cudaStream_t stream) const {
+    int stencil(int epi, int from, void* dst, double omega, double beta, cudaStream_t stream) const override {
         TmaStepParams<T> p;
         p.L = L; p.dst = (T*)dst; p.omega = T(omega); p.lz = lz; p.beta = T(beta);
         if (epi == EPI_SFORM) kernel<EPI_SFORM>()<<<grid, C::NT + 32, C::SMEM, stream>>>(main_map[from], row_map[from], p);
@@ -182,13 +191,19 @@ struct Tma2fPlan {
     }
 
     // gradient pass on one state buffer: fields 12..15 from field 10
-    int normals(void* state, double A, cudaStream_t stream) const {
+    int normals(void* state, double A, cudaStream_t stream) const override {
         constexpr int ZC = 4;
         Normal2Params<T> a;
         a.L = L; a.state = (T*)state; a.A = T(A);
         const int bx = L.nx >= 128 ? 128 : (L.nx >= 64 ? 64 : 32), by = 256 / bx;
         const dim3 b(bx, by, 1), g((L.nx + bx - 1) / bx, (L.ny + by - 1) / by, (L.nz + ZC - 1) / ZC);
-        k_colour_normal<T, ZC><<<g, b, 0, stream>>>(a);
+        k_colour_normal<T, Q, ZC><<<g, b, 0, stream>>>(a);
+        return (int)cudaGetLastError();
+    }
+
+    int import_state(const void* ext, void* state, void* raw, double omega, double beta, cudaStream_t stream) const override {
+        const dim3 b(32, 8, 1), g((L.nx + 31) / 32, (L.ny + 7) / 8, L.nz);
+        k_tma2f_import<T, Q><<<g, b, 0, stream>>>(L, (const T*)ext, (T*)state, (T*)raw, T(omega), T(beta));
         return (int)cudaGetLastError();
     }
 };

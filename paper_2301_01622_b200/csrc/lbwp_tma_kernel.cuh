@@ -125,12 +125,12 @@ __device__ __forceinline__ void store_raw2_node(const XLayout& L, T* __restrict_
 }
 
 // Fused two-component mode (C::NC == 3): finished sums (drho, j, dP_aa, P_ab, rhoA) -> the twelve state fields
-// S-form after BGK (Eq. 8, no perturbation yet), rA = rhoA/rho, kappa = beta rhoA rhoB/rho (x 1/216); the
+// S-form after BGK (Eq. 8, no perturbation yet), rA = rhoA/rho, kappa = beta rhoA rhoB/rho (x 1/216 or 1/36); the
 // interface fields 12..15 are written by the gradient pass (lbwp_tma2f.cuh).
-template <typename T>
+template <typename T, int Q>
 __device__ __forceinline__ void store_state2f(const XLayout& L, T* __restrict__ dst, const T (&a)[11], T omega, T beta, int x,
                                               int y, int z) {
-    const T c = T(1.0 / 216.0);
+    const T c = Q == 27 ? T(1.0 / 216.0) : T(1.0 / 36.0);
     const T rho = T(1) + a[0];
     const T irho = rcp_t<T>(rho);
     const T ux = a[1] * irho, uy = a[2] * irho, uz = a[3] * irho;
@@ -306,7 +306,8 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
             P[f] = P[f] + Cc[f];
         }
 #else
-        if constexpr (C::NC == 3) S::consume2f(sm, rs, P, Cc, N);
+        if constexpr (C::NC == 3 && C::Q == 27) S::consume2f(sm, rs, P, Cc, N);
+        else if constexpr (C::NC == 3) S::consume2f19(sm, rs, P, Cc, N);
         else if constexpr (C::NC == 2 && C::Q == 27) S::consume2c(sm, rs, P, Cc, N);
         else if constexpr (C::NC == 2) S::consume2c19(sm, rs, P, Cc, N);
         else if constexpr (C::Q == 27) S::consume(sm, rs, P, Cc, N);
@@ -325,7 +326,7 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
 #pragma unroll
                     for (int f = 0; f < C::NA; ++f) acc[f] = P[f].get(n);
                     if (EPI == EPI_SFORM)
-                        store_state2f<T>(L, p.dst, acc, p.omega, p.beta, ct.x0 + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
+                        store_state2f<T, C::Q>(L, p.dst, acc, p.omega, p.beta, ct.x0 + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
                     else
                         store_dense2<T>(L, p.dst, acc, ct.x0 + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
                 }

@@ -537,6 +537,71 @@ struct TmaStep {
         N[10] = (maw + mao) + (tin + tz);
         P[10] = P[10] + ((maw - mao) + (tin - tz));
     }
+
+    // Fused two-component mode on D3Q19: brackets and perturbation as above (no z-dependent parts at the in-plane
+    // corners), sums with the D3Q19 weights x 36 as in consume2c19; rest population (A/3)|G| = 24 gh.
+    __device__ static __forceinline__ void consume2f19(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
+                                                       V (&Cc)[C::NA], V (&N)[C::NA]) {
+        const V two = V::bc(T(2)), eight = V::bc(T(8));
+        const V cc = V::bc(T(1.0 / 36.0));
+        V El[3], Wl[3], Ol[3], Em[3], Wm[3], Om[3], Eh[3], Wh[3], Oh[3];
+        V ral[3], ram[3], rah[3], kxl[3], kxm[3], kxh[3], kyl[3], kym[3], kyh[3], kzl[3], kzm[3], kzh[3], ghc, ghu;
+#pragma unroll
+        for (int k = 0; k < 3; k += 2) { Wl[k] = Ol[k] = Wh[k] = Oh[k] = V::bc(T(0)); }   // no such directions
+        brackets<-1, false>(s, r, El, Wl, Ol);
+        colour_fold<-1>(s, r, El, Wl, Ol, ral, kxl, kyl, kzl, ghu);
+        brackets<1, false>(s, r, Eh, Wh, Oh);
+        colour_fold<1>(s, r, Eh, Wh, Oh, rah, kxh, kyh, kzh, ghu);
+        brackets<0, false>(s, r, Em, Wm, Om);
+        colour_fold<0>(s, r, Em, Wm, Om, ram, kxm, kym, kzm, ghc);
+        {   // total fluid: identical to consume19()
+            const XRow<V> xl = xpass<V>(El[0], El[1], El[2], two), xm = xpass<V>(Em[0], Em[1], Em[2], two),
+                          xh = xpass<V>(Eh[0], Eh[1], Eh[2], two);
+            Mom6<V> me = ypass<V>(xl, xm, xh, two);
+            me.m00 = vfma(eight, Em[1], me.m00);
+            Cc[0] = Cc[0] + me.m00; Cc[1] = Cc[1] + me.m10; Cc[2] = Cc[2] + me.m01;
+            Cc[4] = Cc[4] + me.m20; Cc[5] = Cc[5] + me.m02; Cc[7] = Cc[7] + me.m11;
+            const V wx = Wm[2] + Wm[0], wy = Wh[1] + Wl[1], ox = Om[2] + Om[0], oy = Oh[1] + Ol[1];
+            const V w00 = vfma(two, Wm[1], wx + wy), o00 = vfma(two, Om[1], ox + oy);
+            const V w10 = Wm[2] - Wm[0], o10 = Om[2] - Om[0];
+            const V w01 = Wh[1] - Wl[1], o01 = Oh[1] - Ol[1];
+            const V p00 = w00 + o00, p10 = w10 + o10, p01 = w01 + o01;
+            N[0] = p00; N[1] = p10; N[2] = p01; N[3] = p00;
+            N[4] = wx + ox; N[5] = wy + oy; N[6] = p00;
+            N[7] = V::bc(T(0)); N[8] = p10; N[9] = p01;
+            const V n00 = w00 - o00, n10 = w10 - o10, n01 = w01 - o01;
+            P[0] = P[0] + n00; P[1] = P[1] + n10; P[2] = P[2] + n01; P[3] = P[3] - n00;
+            P[4] = P[4] + (wx - ox); P[5] = P[5] + (wy - oy); P[6] = P[6] + n00;
+            P[8] = P[8] - n10; P[9] = P[9] - n01;
+        }
+        // colour A, first part: sum_c w_c rA (1 + B_c) with the perturbed brackets
+        auto ae_of = [&](const V& ra, const V& E) { return vfma(ra, E, ra * cc); };
+        const V rl = vfma(two, ae_of(ral[1], El[1]), ae_of(ral[2], El[2]) + ae_of(ral[0], El[0]));
+        const V aem1 = ae_of(ram[1], Em[1]);
+        const V rm = vfma(two, aem1, ae_of(ram[2], Em[2]) + ae_of(ram[0], Em[0]));
+        const V rh = vfma(two, ae_of(rah[1], Eh[1]), ae_of(rah[2], Eh[2]) + ae_of(rah[0], Eh[0]));
+        const V mae = vfma(eight, aem1, vfma(two, rm, rh + rl));
+        const V maw = vfma(two, ae_of(ram[1], Wm[1]),
+                           (ae_of(ram[2], Wm[2]) + ae_of(ram[0], Wm[0])) + (ae_of(rah[1], Wh[1]) + ae_of(ral[1], Wl[1])));
+        const V mao = vfma(two, ram[1] * Om[1], (ram[2] * Om[2] + ram[0] * Om[0]) + (rah[1] * Oh[1] + ral[1] * Ol[1]));
+        // second part: sum_{c != 0} w_c K.c / |c|; weights x 36 / |c|: 2 (axis), 1/sqrt2 (face diagonal)
+        const V kxa = kxm[2] - kxm[0];
+        const V kxb = (kxh[2] - kxh[0]) + (kxl[2] - kxl[0]);
+        const V kya = kyh[1] - kyl[1];
+        const V kyb = (kyh[2] - kyl[2]) + (kyh[0] - kyl[0]);
+        const V z0 = kzm[1];
+        const V z1 = (kzm[2] + kzm[0]) + (kzh[1] + kzl[1]);
+        const V da = kxa + kya, db = kxb + kyb;
+        const V f2 = V::bc(T(0.70710678118654752));
+        const V t0 = vfma(two, da, f2 * db);
+        const V tin = f2 * da;
+        const V tz = vfma(two, z0, f2 * z1);
+        const V r0 = V::bc(T(24)) * ghc;   // (A/3)|G| in population units
+        Cc[0] = Cc[0] + r0;
+        Cc[10] = (Cc[10] + mae) + vfma(ram[1], r0, t0);
+        N[10] = (maw + mao) + (tin + tz);
+        P[10] = P[10] + ((maw - mao) + (tin - tz));
+    }
 };
 
 }  // namespace lbwp

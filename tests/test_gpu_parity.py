@@ -183,7 +183,7 @@ def test_config3_scaled_droplets(lbwp, oracle, dtype, lattice):
 @pytest.mark.parametrize("dtype,shape", [("f32", (64, 24, 20)), ("f32", (128, 16, 37)), ("f32", (64, 8, 2)),
                                          ("f64", (32, 24, 20)), ("f64", (64, 16, 5))])
 @pytest.mark.parametrize("steps,tau", [(1, 1.0), (30, 0.7)])
-@pytest.mark.parametrize("lattice,kernel", [(27, "tma"), (27, "tma_split"), (19, "tma")])
+@pytest.mark.parametrize("lattice,kernel", [(27, "tma"), (27, "tma_split"), (19, "tma"), (19, "tma_split")])
 def test_tma_two_component(lbwp, oracle, dtype, shape, steps, tau, lattice, kernel):
     nx, ny, nz = shape
     tg = wl.taylor_green(0, shape=shape)
@@ -192,7 +192,7 @@ def test_tma_two_component(lbwp, oracle, dtype, shape, steps, tau, lattice, kern
     cfg = dict(name="tma2_q%d_%s_%s" % (lattice, dtype, "x".join(map(str, shape))), moments=m, lattice=lattice, ncomp=2,
                tau=tau, A=0.01, beta=0.7, dtype=dtype)
     m0 = wl.as_dtype(m, dtype)
-    split = kernel == "tma_split" or lattice == 19
+    split = kernel == "tma_split"
     with lbwp.Lbwp(m0, lattice=lattice, dtype=dtype, ncomp=2, tau=tau, A=0.01, beta=0.7, kernel=kernel) as sim:
         assert sim.kernel_name == "tma%d_%s_c2%s" % (lattice, dtype, "split" if split else "")
         assert sim.launches_per_step == 2
