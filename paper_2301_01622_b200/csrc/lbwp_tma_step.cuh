@@ -465,25 +465,51 @@ struct TmaStep {
         }
     }
 
+    // one source row of the fused two-component plane, reduced at once to what the plane sums need (keeps the
+    // live set small: the kernel runs at its register limit)
+    struct Row2f {
+        XRow<V> e, w, o;          // x-pass of the perturbed brackets
+        V ae, aw, ao;             // x-pass (zeroth moment) of rA (1 + bracket)
+        V kxd, kyc, kys, kzc, kzs;  // Kx(+1) - Kx(-1); Ky, Kz at cx = 0; their sums over cx = +-1
+    };
+    template <int CY>
+    __device__ static __forceinline__ void row2f(const T* __restrict__ s, const int (&r)[C::NPT][3], const V& four, const V& cc,
+                                                 Row2f& out, V& gh_mid) {
+        V E[3], W[3], O[3], ra[3], kx[3], ky[3], kz[3];
+        brackets<CY, true>(s, r, E, W, O);
+        colour_fold<CY>(s, r, E, W, O, ra, kx, ky, kz, gh_mid);
+        out.e = xpass<V>(E[0], E[1], E[2], four);
+        out.w = xpass<V>(W[0], W[1], W[2], four);
+        out.o = xpass<V>(O[0], O[1], O[2], four);
+        V AE[3], AW[3], AO[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const V rac = ra[k] * cc;
+            AE[k] = vfma(ra[k], E[k], rac);
+            AW[k] = vfma(ra[k], W[k], rac);
+            AO[k] = ra[k] * O[k];
+        }
+        out.ae = vfma(four, AE[1], AE[2] + AE[0]);
+        out.aw = vfma(four, AW[1], AW[2] + AW[0]);
+        out.ao = vfma(four, AO[1], AO[2] + AO[0]);
+        out.kxd = kx[2] - kx[0];
+        out.kyc = ky[1]; out.kys = ky[2] + ky[0];
+        out.kzc = kz[1]; out.kzs = kz[2] + kz[0];
+    }
+
     __device__ static __forceinline__ void consume2f(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
                                                      V (&Cc)[C::NA], V (&N)[C::NA]) {
         const V four = V::bc(T(4));
         const V cc = V::bc(T(1.0 / 216.0));
-        V El[3], Wl[3], Ol[3], Em[3], Wm[3], Om[3], Eh[3], Wh[3], Oh[3];
-        V ral[3], ram[3], rah[3], kxl[3], kxm[3], kxh[3], kyl[3], kym[3], kyh[3], kzl[3], kzm[3], kzh[3], ghc, ghu;
-        brackets<-1, true>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
-        colour_fold<-1>(s, r, El, Wl, Ol, ral, kxl, kyl, kzl, ghu);
-        brackets<1, true>(s, r, Eh, Wh, Oh);    // sources at y-1 (cy = +1)
-        colour_fold<1>(s, r, Eh, Wh, Oh, rah, kxh, kyh, kzh, ghu);
-        brackets<0, true>(s, r, Em, Wm, Om);
-        colour_fold<0>(s, r, Em, Wm, Om, ram, kxm, kym, kzm, ghc);
+        Row2f l, m, h;
+        V ghc, ghu;
+        row2f<-1>(s, r, four, cc, l, ghu);   // sources at y+1 (cy = -1)
+        row2f<1>(s, r, four, cc, h, ghu);    // sources at y-1 (cy = +1)
+        row2f<0>(s, r, four, cc, m, ghc);
         {   // total fluid: identical to consume()
-            const Mom6<V> me = ypass<V>(xpass<V>(El[0], El[1], El[2], four), xpass<V>(Em[0], Em[1], Em[2], four),
-                                        xpass<V>(Eh[0], Eh[1], Eh[2], four), four);
-            const Mom6<V> mw = ypass<V>(xpass<V>(Wl[0], Wl[1], Wl[2], four), xpass<V>(Wm[0], Wm[1], Wm[2], four),
-                                        xpass<V>(Wh[0], Wh[1], Wh[2], four), four);
-            const Mom6<V> mo = ypass<V>(xpass<V>(Ol[0], Ol[1], Ol[2], four), xpass<V>(Om[0], Om[1], Om[2], four),
-                                        xpass<V>(Oh[0], Oh[1], Oh[2], four), four);
+            const Mom6<V> me = ypass<V>(l.e, m.e, h.e, four);
+            const Mom6<V> mw = ypass<V>(l.w, m.w, h.w, four);
+            const Mom6<V> mo = ypass<V>(l.o, m.o, h.o, four);
             Cc[0] = vfma(four, me.m00, Cc[0]);
             Cc[1] = vfma(four, me.m10, Cc[1]);
             Cc[2] = vfma(four, me.m01, Cc[2]);
@@ -499,41 +525,21 @@ struct TmaStep {
             P[4] = P[4] + (mw.m20 - mo.m20); P[5] = P[5] + (mw.m02 - mo.m02); P[6] = P[6] + n00;
             P[7] = P[7] + (mw.m11 - mo.m11); P[8] = P[8] - n10; P[9] = P[9] - n01;
         }
-        // colour A, first part: sum_c w_c rA (1 + B_c) with the perturbed brackets; zeroth in-plane moment only
-        auto a_row = [&](const V (&ra)[3], const V (&E)[3], const V (&W)[3], const V (&O)[3], V& ae, V& aw, V& ao) {
-            V AE[3], AW[3], AO[3];
-#pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                const V rac = ra[k] * cc;
-                AE[k] = vfma(ra[k], E[k], rac);
-                AW[k] = vfma(ra[k], W[k], rac);
-                AO[k] = ra[k] * O[k];
-            }
-            ae = vfma(four, AE[1], AE[2] + AE[0]);
-            aw = vfma(four, AW[1], AW[2] + AW[0]);
-            ao = vfma(four, AO[1], AO[2] + AO[0]);
-        };
-        V ael, awl, aol, aem, awm, aom, aeh, awh, aoh;
-        a_row(ral, El, Wl, Ol, ael, awl, aol);
-        a_row(rah, Eh, Wh, Oh, aeh, awh, aoh);
-        a_row(ram, Em, Wm, Om, aem, awm, aom);
-        const V mae = vfma(four, aem, aeh + ael), maw = vfma(four, awm, awh + awl), mao = vfma(four, aom, aoh + aol);
+        // colour A, first part: sum_c w_c rA (1 + B_c) with the perturbed brackets
+        const V mae = vfma(four, m.ae, h.ae + l.ae), maw = vfma(four, m.aw, h.aw + l.aw), mao = vfma(four, m.ao, h.ao + l.ao);
         // second part: sum_{c != 0} w_c K.c / |c|; weights x 216 / |c|: 16 (axis), 4/sqrt2 (face), 1/sqrt3 (corner)
-        const V kxa = kxm[2] - kxm[0];
-        const V kxb = (kxh[2] - kxh[0]) + (kxl[2] - kxl[0]);
-        const V kya = kyh[1] - kyl[1];
-        const V kyb = (kyh[2] - kyl[2]) + (kyh[0] - kyl[0]);
-        const V z0 = kzm[1];
-        const V z1 = (kzm[2] + kzm[0]) + (kzh[1] + kzl[1]);
-        const V z2 = (kzh[2] + kzh[0]) + (kzl[2] + kzl[0]);
-        const V da = kxa + kya, db = kxb + kyb;
+        const V da = m.kxd + (h.kyc - l.kyc);
+        const V db = (h.kxd + l.kxd) + (h.kys - l.kys);
+        const V z1 = m.kzs + (h.kzc + l.kzc);
+        const V z2 = h.kzs + l.kzs;
         const V f1 = V::bc(T(16)), f2 = V::bc(T(2.8284271247461903)), f3 = V::bc(T(0.57735026918962576));
         const V t0 = vfma(f1, da, f2 * db);
         const V tin = vfma(f2, da, f3 * db);
-        const V tz = vfma(f1, z0, vfma(f2, z1, f3 * z2));
+        const V tz = vfma(f1, m.kzc, vfma(f2, z1, f3 * z2));
         const V r0 = V::bc(T(144)) * ghc;   // (A/3)|G| in population units
         Cc[0] = Cc[0] + r0;
-        Cc[10] = vfma(four, mae, Cc[10]) + vfma(ram[1], r0, t0);
+        // rA of the node itself: recomputed load (cheaper than keeping it live across the rows)
+        Cc[10] = vfma(four, mae, Cc[10]) + vfma(ld<10, 0>(s, r, 1), r0, t0);
         N[10] = (maw + mao) + (tin + tz);
         P[10] = P[10] + ((maw - mao) + (tin - tz));
     }
