@@ -212,6 +212,15 @@ def test_config3_full_size(lbwp, oracle):
     assert agree >= 0.9999
 
 
+# ---- config 4 (256^3 off-axis collision, fp32): its 4000 steps are hours of oracle time, so the full-size box is
+#      checked over its first steps (12; 100 with LBWP_FULL_CONFIGS=1) in the launch configuration bench.py times ----
+def test_config4_full_size_first_steps(lbwp, oracle):
+    cfg = wl.config4(256)
+    got, ref = check(lbwp, oracle, cfg, 100 if FULL else 12)
+    agree = np.mean(np.sign(got[0].astype(np.float64) - got[1]) == np.sign(ref[0] - ref[1]))
+    assert agree >= 0.9999
+
+
 # ---- comparison kernel vs its own mini-oracle (population-storing pull BGK) ----------------
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 @pytest.mark.parametrize("lattice", [19, 27])
