@@ -131,7 +131,7 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def time_oracle(a, seconds_target=15.0):
+def time_oracle(a, seconds_target=20.0):
     """The oracle as it stands on the host cores: bounded sample of the workload's recipe."""
     import oracle
     from paper_2301_01622_b200 import workloads as wl
