@@ -544,33 +544,63 @@ struct TmaStep {
         P[10] = P[10] + ((maw - mao) + (tin - tz));
     }
 
+    // D3Q19 row of the fused two-component plane, reduced at once (cf. Row2f).  SIDES: the row cy = 0, which also
+    // carries the off-plane directions (+-1, 0, cz); rows cy = +-1 carry them at cx = 0 only.
+    struct Row2f19 {
+        XRow<V> e;                   // (1,2,1) x-pass of the perturbed E brackets
+        V e1;                        // E at cx = 0 (extra centre weight), row cy = 0 only
+        V w1, o1, ws, wd, os, od;    // W, O at cx = 0; sum / difference over cx = +-1 (row cy = 0 only)
+        V ae, ae1, aw1, ao1, aws, aos;   // the same for rA (1 + bracket)
+        V kxd, kyc, kys, kzc, kzs;
+    };
+    template <int CY>
+    __device__ static __forceinline__ void row2f19(const T* __restrict__ s, const int (&r)[C::NPT][3], const V& two, const V& cc,
+                                                   Row2f19& out, V& gh_mid) {
+        constexpr bool SIDES = CY == 0;
+        V E[3], W[3], O[3], ra[3], kx[3], ky[3], kz[3];
+        W[0] = W[2] = O[0] = O[2] = V::bc(T(0));   // no such directions on rows cy = +-1
+        brackets<CY, false>(s, r, E, W, O);
+        colour_fold<CY>(s, r, E, W, O, ra, kx, ky, kz, gh_mid);
+        out.e = xpass<V>(E[0], E[1], E[2], two);
+        V AE[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) AE[k] = vfma(ra[k], E[k], ra[k] * cc);
+        out.ae = vfma(two, AE[1], AE[2] + AE[0]);
+        out.w1 = W[1]; out.o1 = O[1];
+        out.aw1 = vfma(ra[1], W[1], ra[1] * cc);
+        out.ao1 = ra[1] * O[1];
+        if (SIDES) {
+            out.e1 = E[1]; out.ae1 = AE[1];
+            out.ws = W[2] + W[0]; out.wd = W[2] - W[0];
+            out.os = O[2] + O[0]; out.od = O[2] - O[0];
+            out.aws = vfma(ra[2], W[2], ra[2] * cc) + vfma(ra[0], W[0], ra[0] * cc);
+            out.aos = ra[2] * O[2] + ra[0] * O[0];
+        }
+        out.kxd = kx[2] - kx[0];
+        out.kyc = ky[1]; out.kys = ky[2] + ky[0];
+        out.kzc = kz[1]; out.kzs = kz[2] + kz[0];
+    }
+
     // Fused two-component mode on D3Q19: brackets and perturbation as above (no z-dependent parts at the in-plane
     // corners), sums with the D3Q19 weights x 36 as in consume2c19; rest population (A/3)|G| = 24 gh.
     __device__ static __forceinline__ void consume2f19(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
                                                        V (&Cc)[C::NA], V (&N)[C::NA]) {
         const V two = V::bc(T(2)), eight = V::bc(T(8));
         const V cc = V::bc(T(1.0 / 36.0));
-        V El[3], Wl[3], Ol[3], Em[3], Wm[3], Om[3], Eh[3], Wh[3], Oh[3];
-        V ral[3], ram[3], rah[3], kxl[3], kxm[3], kxh[3], kyl[3], kym[3], kyh[3], kzl[3], kzm[3], kzh[3], ghc, ghu;
-#pragma unroll
-        for (int k = 0; k < 3; k += 2) { Wl[k] = Ol[k] = Wh[k] = Oh[k] = V::bc(T(0)); }   // no such directions
-        brackets<-1, false>(s, r, El, Wl, Ol);
-        colour_fold<-1>(s, r, El, Wl, Ol, ral, kxl, kyl, kzl, ghu);
-        brackets<1, false>(s, r, Eh, Wh, Oh);
-        colour_fold<1>(s, r, Eh, Wh, Oh, rah, kxh, kyh, kzh, ghu);
-        brackets<0, false>(s, r, Em, Wm, Om);
-        colour_fold<0>(s, r, Em, Wm, Om, ram, kxm, kym, kzm, ghc);
+        Row2f19 l, m, h;
+        V ghc, ghu;
+        row2f19<-1>(s, r, two, cc, l, ghu);
+        row2f19<1>(s, r, two, cc, h, ghu);
+        row2f19<0>(s, r, two, cc, m, ghc);
         {   // total fluid: identical to consume19()
-            const XRow<V> xl = xpass<V>(El[0], El[1], El[2], two), xm = xpass<V>(Em[0], Em[1], Em[2], two),
-                          xh = xpass<V>(Eh[0], Eh[1], Eh[2], two);
-            Mom6<V> me = ypass<V>(xl, xm, xh, two);
-            me.m00 = vfma(eight, Em[1], me.m00);
+            Mom6<V> me = ypass<V>(l.e, m.e, h.e, two);
+            me.m00 = vfma(eight, m.e1, me.m00);
             Cc[0] = Cc[0] + me.m00; Cc[1] = Cc[1] + me.m10; Cc[2] = Cc[2] + me.m01;
             Cc[4] = Cc[4] + me.m20; Cc[5] = Cc[5] + me.m02; Cc[7] = Cc[7] + me.m11;
-            const V wx = Wm[2] + Wm[0], wy = Wh[1] + Wl[1], ox = Om[2] + Om[0], oy = Oh[1] + Ol[1];
-            const V w00 = vfma(two, Wm[1], wx + wy), o00 = vfma(two, Om[1], ox + oy);
-            const V w10 = Wm[2] - Wm[0], o10 = Om[2] - Om[0];
-            const V w01 = Wh[1] - Wl[1], o01 = Oh[1] - Ol[1];
+            const V wx = m.ws, wy = h.w1 + l.w1, ox = m.os, oy = h.o1 + l.o1;
+            const V w00 = vfma(two, m.w1, wx + wy), o00 = vfma(two, m.o1, ox + oy);
+            const V w10 = m.wd, o10 = m.od;
+            const V w01 = h.w1 - l.w1, o01 = h.o1 - l.o1;
             const V p00 = w00 + o00, p10 = w10 + o10, p01 = w01 + o01;
             N[0] = p00; N[1] = p10; N[2] = p01; N[3] = p00;
             N[4] = wx + ox; N[5] = wy + oy; N[6] = p00;
@@ -581,30 +611,20 @@ struct TmaStep {
             P[8] = P[8] - n10; P[9] = P[9] - n01;
         }
         // colour A, first part: sum_c w_c rA (1 + B_c) with the perturbed brackets
-        auto ae_of = [&](const V& ra, const V& E) { return vfma(ra, E, ra * cc); };
-        const V rl = vfma(two, ae_of(ral[1], El[1]), ae_of(ral[2], El[2]) + ae_of(ral[0], El[0]));
-        const V aem1 = ae_of(ram[1], Em[1]);
-        const V rm = vfma(two, aem1, ae_of(ram[2], Em[2]) + ae_of(ram[0], Em[0]));
-        const V rh = vfma(two, ae_of(rah[1], Eh[1]), ae_of(rah[2], Eh[2]) + ae_of(rah[0], Eh[0]));
-        const V mae = vfma(eight, aem1, vfma(two, rm, rh + rl));
-        const V maw = vfma(two, ae_of(ram[1], Wm[1]),
-                           (ae_of(ram[2], Wm[2]) + ae_of(ram[0], Wm[0])) + (ae_of(rah[1], Wh[1]) + ae_of(ral[1], Wl[1])));
-        const V mao = vfma(two, ram[1] * Om[1], (ram[2] * Om[2] + ram[0] * Om[0]) + (rah[1] * Oh[1] + ral[1] * Ol[1]));
+        const V mae = vfma(eight, m.ae1, vfma(two, m.ae, h.ae + l.ae));
+        const V maw = vfma(two, m.aw1, m.aws + (h.aw1 + l.aw1));
+        const V mao = vfma(two, m.ao1, m.aos + (h.ao1 + l.ao1));
         // second part: sum_{c != 0} w_c K.c / |c|; weights x 36 / |c|: 2 (axis), 1/sqrt2 (face diagonal)
-        const V kxa = kxm[2] - kxm[0];
-        const V kxb = (kxh[2] - kxh[0]) + (kxl[2] - kxl[0]);
-        const V kya = kyh[1] - kyl[1];
-        const V kyb = (kyh[2] - kyl[2]) + (kyh[0] - kyl[0]);
-        const V z0 = kzm[1];
-        const V z1 = (kzm[2] + kzm[0]) + (kzh[1] + kzl[1]);
-        const V da = kxa + kya, db = kxb + kyb;
+        const V da = m.kxd + (h.kyc - l.kyc);
+        const V db = (h.kxd + l.kxd) + (h.kys - l.kys);
+        const V z1 = m.kzs + (h.kzc + l.kzc);
         const V f2 = V::bc(T(0.70710678118654752));
         const V t0 = vfma(two, da, f2 * db);
         const V tin = f2 * da;
-        const V tz = vfma(two, z0, f2 * z1);
+        const V tz = vfma(two, m.kzc, f2 * z1);
         const V r0 = V::bc(T(24)) * ghc;   // (A/3)|G| in population units
         Cc[0] = Cc[0] + r0;
-        Cc[10] = (Cc[10] + mae) + vfma(ram[1], r0, t0);
+        Cc[10] = (Cc[10] + mae) + vfma(ld<10, 0>(s, r, 1), r0, t0);
         N[10] = (maw + mao) + (tin + tz);
         P[10] = P[10] + ((maw - mao) + (tin - tz));
     }
