@@ -203,13 +203,49 @@ def test_tma_two_component(lbwp, oracle, dtype, shape, steps, tau, lattice, kern
     assert agree >= 0.9999
 
 
-# ---- config 3 itself (128^3, fp32, tau=1, A=0.01, beta=0.7); 40 steps by default (oracle time),
-#      the full 2000 with LBWP_FULL_CONFIGS=1 ---
+# ---- config 3 itself (128^3, fp32, tau=1, A=0.01, beta=0.7).  The drops touch between steps 100 and 200 and the
+#      rupture of the film between them amplifies any perturbation by 1e4-1e5 (measured: the fp64 kernel goes from
+#      7e-14 to 4e-10 against the fp64 oracle, three independent fp32 kernels from 3e-6 to 0.1-0.18, and 0.06 apart from
+#      each other: profiles/r01_config3_divergence.md).  BASELINE's fp32 tolerance is therefore gated up to the contact;
+#      after it (LBWP_FULL_CONFIGS=1: all 2000 steps) the gates are what an fp32 trajectory can keep: colour masses, the
+#      sign of the phase field on >= 99.9 % of the nodes, bounded fields.  The fp64 run of the same configuration must
+#      stay within 2e-5 and 100 % sign agreement through the collision (next test). ---
 def test_config3_full_size(lbwp, oracle):
     cfg = wl.config3(128)
-    got, ref = check(lbwp, oracle, cfg, 2000 if FULL else 40)
-    agree = np.mean(np.sign(got[0].astype(np.float64) - got[1]) == np.sign(ref[0] - ref[1]))
-    assert agree >= 0.9999
+    m0 = wl.as_dtype(cfg["moments"], "f32")
+    kw = dict(lattice=27, ncomp=2, tau=cfg["tau"], A=cfg["A"], beta=cfg["beta"])
+    pre = 100 if FULL else 40
+    with lbwp.Lbwp(m0, dtype="f32", **kw) as sim:
+        sim.step(pre)
+        got = sim.moments_host()
+        ref = oracle.run(m0, nsteps=pre, **kw)
+        assert parity_errors(got, ref, 2, "f32").max() <= TOL["f32"]
+        assert np.mean(np.sign(got[0].astype(np.float64) - got[1]) == np.sign(ref[0] - ref[1])) >= 0.9999
+        if not FULL:
+            return
+        sim.step(2000 - pre)
+        got = sim.moments_host().astype(np.float64)
+    ref = oracle.run(ref, nsteps=2000 - pre, **kw)
+    assert np.isfinite(got).all() and np.abs(got[2:5]).max() < 0.2
+    for k in (0, 1):                                   # each colour's mass (Eq. 1 summed over the box)
+        assert abs(got[k].sum() - m0[k].astype(np.float64).sum()) <= 2e-5 * m0[k].astype(np.float64).sum()
+    assert np.mean(np.sign(got[0] - got[1]) == np.sign(ref[0] - ref[1])) >= 0.999
+    print("config3 after 2000 steps, fp32 vs fp64 oracle:", parity_errors(got, ref, 2, "f32"))
+
+
+def test_config3_long_run_fp64(lbwp, oracle):
+    """Same configuration in fp64, through the collision (300 steps; 2000 with LBWP_FULL_CONFIGS=1): the kernel differs
+    from the oracle only in the order of its additions, and even that is amplified to 1e-6 (never beyond 2e-5)."""
+    cfg = wl.config3(128)
+    m0 = wl.as_dtype(cfg["moments"], "f32").astype(np.float64)
+    kw = dict(lattice=27, ncomp=2, tau=cfg["tau"], A=cfg["A"], beta=cfg["beta"])
+    steps = 2000 if FULL else 300
+    with lbwp.Lbwp(m0, dtype="f64", **kw) as sim:
+        sim.step(steps)
+        got = sim.moments_host()
+    ref = oracle.run(m0, nsteps=steps, **kw)
+    assert parity_errors(got, ref, 2, "f64").max() <= 2e-5
+    assert np.mean(np.sign(got[0] - got[1]) == np.sign(ref[0] - ref[1])) == 1.0
 
 
 # ---- config 4 (256^3 off-axis collision, fp32): its 4000 steps are hours of oracle time, so the full-size box is
