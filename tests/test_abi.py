@@ -64,6 +64,29 @@ def test_invalid_params_rejected(lib, bad):
     assert b"invalid" in lib.lbwp_last_error()
 
 
+def test_unbuilt_kernel_combinations_rejected(lib):
+    """A kernel variant asked for a combination it is not built for: LBWP_EUNSUPPORTED, before any CUDA call."""
+    cases = [dict(kernel="tma", shape=(8, 8, 40)),                      # tiles do not divide the box
+             dict(kernel="tma_split", ncomp=1, shape=(8, 8, 64)),        # split form is two-component only
+             dict(kernel="march", lattice=19, shape=(8, 8, 8)),
+             dict(kernel="march", ncomp=2, shape=(8, 8, 8))]
+    for c in cases:
+        kw = dict(lattice=27, dtype="f32", ncomp=1, tau=0.8)
+        kw.update(c)
+        p = lbwp.make_params(**kw)
+        assert lbwp.state_bytes(p) == 0
+        ctx = ctypes.c_void_p()
+        buf = (ctypes.c_float * (11 * 8 * 8 * 64))()
+        rc = lib.lbwp_init(ctypes.byref(p), buf, 0, ctypes.byref(ctx))
+        assert rc == -4 and not ctx.value, c
+    # the TMA variants size their state by what they keep: 10 fields, or 16 for two components
+    p1 = lbwp.make_params(lattice=27, dtype="f32", ncomp=1, shape=(64, 64, 128), tau=0.8, kernel="tma")
+    p2 = lbwp.make_params(lattice=27, dtype="f32", ncomp=2, shape=(64, 64, 128), tau=0.8, kernel="tma")
+    p3 = lbwp.make_params(lattice=19, dtype="f32", ncomp=2, shape=(64, 64, 128), tau=0.8, kernel="tma_split")
+    b1, b2, b3 = (lbwp.state_bytes(p) for p in (p1, p2, p3))
+    assert b1 == 10 * 4 * 64 * 64 * 136 and b2 == 16 * 4 * 64 * 64 * 136 and b3 == 15 * 4 * 64 * 64 * 136
+
+
 def test_no_cpu_fallback(lib):
     """Without a GPU lbwp_init must fail loudly, not compute on the host."""
     import torch
