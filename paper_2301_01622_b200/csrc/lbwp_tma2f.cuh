@@ -36,21 +36,20 @@ __global__ void __launch_bounds__(256) k_colour_normal(const Normal2Params<T> p)
     if (x >= L.nx || y >= L.ny) return;
     const long long F = L.field;
     const T* __restrict__ ra = p.state + 10 * F;
-    const int xs[3] = {x == 0 ? L.nx - 1 : x - 1, x, x == L.nx - 1 ? 0 : x + 1};
+    // x neighbours come from the ghost columns the stencil epilogue maintains for rA; y and z wrap here (reading C13)
     const int ys[3] = {y == 0 ? L.ny - 1 : y - 1, y, y == L.ny - 1 ? 0 : y + 1};
-    int off[3][3];
+    int off[3];
 #pragma unroll
-    for (int j = 0; j < 3; ++j)
-#pragma unroll
-        for (int i = 0; i < 3; ++i) off[j][i] = ys[j] * L.px + L.ox + xs[i];
+    for (int j = 0; j < 3; ++j) off[j] = ys[j] * L.px + L.ox + x;
     auto load_plane = [&](int z, T (&f)[3][3]) {
         z = z < 0 ? z + L.nz : z;
         while (z >= L.nz) z -= L.nz;   // planes past a ragged last chunk are loaded (and ignored)
         const T* __restrict__ q = ra + (long long)z * L.plane;
 #pragma unroll
-        for (int j = 0; j < 3; ++j)
-#pragma unroll
-            for (int i = 0; i < 3; ++i) f[j][i] = q[off[j][i]];
+        for (int j = 0; j < 3; ++j) {
+            const T* __restrict__ qr = q + off[j];
+            f[j][0] = qr[-1]; f[j][1] = qr[0]; f[j][2] = qr[1];
+        }
     };
     // all ZC + 2 planes are requested before the first one is used: the pass is latency-bound otherwise
     // (9 loads in flight per thread gave 1.14 ms at 512^3 for 2.7 GB of traffic)
@@ -86,7 +85,7 @@ __global__ void __launch_bounds__(256) k_colour_normal(const Normal2Params<T> p)
         T out[4];
         out[0] = (Q == 27 ? T(1.0 / 216.0) : T(1.0 / 36.0)) * T(0.5) * p.A * g;
         out[1] = gx * ig; out[2] = gy * ig; out[3] = gz * ig;
-        T* __restrict__ d = p.state + 12 * F + (long long)z * L.plane + off[1][1];
+        T* __restrict__ d = p.state + 12 * F + (long long)z * L.plane + off[1];
 #pragma unroll
         for (int f = 0; f < 4; ++f) d[f * F] = out[f];
         if (x == 0 || x == L.nx - 1) {
