@@ -299,6 +299,29 @@ def test_zero_steps_and_round_trip(lbwp):
         assert np.array_equal(sim.moments_host(), b)   # deterministic
 
 
+@pytest.mark.parametrize("ncomp", [1, 2])
+def test_checkpoint_resume(lbwp, ncomp):
+    """The moments are the complete state: lbwp_moments -> lbwp_init continues the run.  The TMA path
+    stores collided moments internally, so a resume re-collides the exported ones: equal up to rounding, not bit for bit."""
+    shape = (64, 16, 12)
+    if ncomp == 1:
+        m0 = wl.noisy_solenoidal(0, shape=shape)
+    else:
+        m0 = wl.droplets(0, [(20, 8, 6), (50, 3, 4)], 5, [0.03, -0.03], shape=shape)
+    kw = dict(lattice=27, dtype="f64", ncomp=ncomp, tau=0.7, A=0.01, beta=0.7)
+    with lbwp.Lbwp(m0, **kw) as sim:
+        assert sim.kernel_name.startswith("tma27")
+        sim.step(8)
+        straight = sim.moments_host()
+    with lbwp.Lbwp(m0, **kw) as sim:
+        sim.step(4)
+        mid = sim.moments_host()
+    with lbwp.Lbwp(mid, **kw) as sim:
+        sim.step(4)
+        resumed = sim.moments_host()
+    assert np.abs(resumed - straight).max() <= 1e-13
+
+
 def test_device_input_and_errors(lbwp):
     import torch
     cfg = wl.config1()
