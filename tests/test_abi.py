@@ -87,6 +87,27 @@ def test_unbuilt_kernel_combinations_rejected(lib):
     assert b1 == 10 * 4 * 64 * 64 * 136 and b2 == 16 * 4 * 64 * 64 * 136 and b3 == 15 * 4 * 64 * 64 * 136
 
 
+def test_paper_array_counts_and_memory(lib):
+    """PAPER.md:75, 163 (tests/golden/paper_arrays_and_memory.txt): 20/22 hydro-arrays against 38/76 population arrays
+    for D3Q19 with Flip-Flop, and a measured saving of 1.1411 - 0.6782 GB at 128^3 two-component single precision."""
+    gold = {}
+    for line in open(os.path.join(ROOT, "tests", "golden", "paper_arrays_and_memory.txt")):
+        line = line.split("#")[0].split()
+        if len(line) == 2:
+            gold[line[0]] = float(line[1])
+    for ncomp, key in ((1, "arrays_moments_1c"), (2, "arrays_moments_2c")):
+        p = lbwp.make_params(lattice=19, dtype="f32", ncomp=ncomp, shape=(128, 128, 128), tau=1.0)
+        assert 2 * lib.lbwp_num_moments(ctypes.byref(p)) == gold[key]
+    assert 2 * 19 * 1 == gold["arrays_populations_1c"] and 2 * 19 * 2 == gold["arrays_populations_2c"]
+    # the saving the array counts predict, against the one the paper measured (whole-process figures): within 3 %
+    predicted = (gold["arrays_populations_2c"] - gold["arrays_moments_2c"]) * 4 * 128 ** 3 / 1e9
+    measured = gold["memory_populations_gb"] - gold["memory_moments_gb"]
+    assert abs(predicted / measured - 1) < 0.03
+    # this library, same case, external accounting: 2 x M x 4 B per node is what the method needs at least
+    p2 = lbwp.make_params(lattice=19, dtype="f32", ncomp=2, shape=(128, 128, 128), tau=1.0)
+    assert 2 * lbwp.state_bytes(p2) >= gold["arrays_moments_2c"] * 4 * 128 ** 3
+
+
 def test_no_cpu_fallback(lib):
     """Without a GPU lbwp_init must fail loudly, not compute on the host."""
     import torch
