@@ -88,7 +88,8 @@ int lbwp_num_moments(const lbwp_params *params);
 /* Create a context and load the initial moments (external layout above; `moments`
  * is a HOST pointer if moments_on_device == 0, else a DEVICE pointer on
  * params->device).  For scheme == LBWP_POPULATIONS the initial populations are the
- * Eq. 4 reconstruction of these moments.  Synchronises the stream
+ * Eq. 4 reconstruction of these moments; with ncomp == 2 one set
+ * per colour, split as f^A = (rho_A / rho) f.  Synchronises the stream
  * before returning.  *out is set only on success. */
 int lbwp_init(const lbwp_params *params, const void *moments, int moments_on_device, lbwp_ctx **out);
 

@@ -131,10 +131,24 @@ struct Ctx final : lbwp_ctx {
         return 0;
     }
 
+    // two-component population step (lbwp_pop.cuh): grad = 3 gradient fields + 2 density fields
+    template <int Q>
+    void step_pop2(const lbwp::StepParams<T>& s) {
+        const dim3 b(32, 8, 1), g = node_grid(L, b);
+        T* dens2 = (T*)grad + 3 * L.field;
+        lbwp::k_pop2_density<T, Q><<<g, b, 0, stream>>>(s, dens2);
+        lbwp::StepParams<T> d = s;
+        d.src = dens2;
+        lbwp::k_colour_gradient<T, Q><<<g, b, 0, stream>>>(d, (T*)grad);
+        lbwp::k_pop2_step<T, Q><<<g, b, 0, stream>>>(s);
+    }
+
     int step_once() override {
         const lbwp::StepParams<T> s = sp(cur, cur ^ 1);
         const dim3 b(32, 8, 1), g = node_grid(L, b);
-        if (P.scheme == LBWP_POPULATIONS) {
+        if (P.scheme == LBWP_POPULATIONS && P.ncomp == 2) {
+            if (P.lattice == 27) step_pop2<27>(s); else step_pop2<19>(s);
+        } else if (P.scheme == LBWP_POPULATIONS) {
             if (P.lattice == 27) lbwp::k_pop_step<T, 27><<<g, b, 0, stream>>>(s);
             else lbwp::k_pop_step<T, 19><<<g, b, 0, stream>>>(s);
         } else {
@@ -154,7 +168,10 @@ struct Ctx final : lbwp_ctx {
         steps = 0;
         if (P.scheme == LBWP_POPULATIONS) {
             // seed F_{-1} in buf[1], then one collide pass gives F_0 in buf[0] (lbwp_pop.cuh)
-            if (P.lattice == 27) lbwp::k_pop_import<T, 27><<<g, b, 0, stream>>>(L, (const T*)ext, (T*)buf[1]);
+            if (P.ncomp == 2) {
+                if (P.lattice == 27) lbwp::k_pop2_import<T, 27><<<g, b, 0, stream>>>(L, (const T*)ext, (T*)buf[1]);
+                else lbwp::k_pop2_import<T, 19><<<g, b, 0, stream>>>(L, (const T*)ext, (T*)buf[1]);
+            } else if (P.lattice == 27) lbwp::k_pop_import<T, 27><<<g, b, 0, stream>>>(L, (const T*)ext, (T*)buf[1]);
             else lbwp::k_pop_import<T, 19><<<g, b, 0, stream>>>(L, (const T*)ext, (T*)buf[1]);
             CU(cudaGetLastError());
             cur = 1;
@@ -172,7 +189,10 @@ struct Ctx final : lbwp_ctx {
     int export_dense(void* ext) override {
         const dim3 b(32, 8, 1), g = node_grid(L, b);
         if (P.scheme == LBWP_POPULATIONS) {
-            if (P.lattice == 27) lbwp::k_pop_export<T, 27><<<g, b, 0, stream>>>(L, (const T*)buf[cur ^ 1], (T*)ext);
+            if (P.ncomp == 2) {
+                if (P.lattice == 27) lbwp::k_pop2_export<T, 27><<<g, b, 0, stream>>>(L, (const T*)buf[cur ^ 1], (T*)ext);
+                else lbwp::k_pop2_export<T, 19><<<g, b, 0, stream>>>(L, (const T*)buf[cur ^ 1], (T*)ext);
+            } else if (P.lattice == 27) lbwp::k_pop_export<T, 27><<<g, b, 0, stream>>>(L, (const T*)buf[cur ^ 1], (T*)ext);
             else lbwp::k_pop_export<T, 19><<<g, b, 0, stream>>>(L, (const T*)buf[cur ^ 1], (T*)ext);
         } else if (P.ncomp == 1) {
             lbwp::k_export_moments<T, 1><<<g, b, 0, stream>>>(L, (const T*)buf[cur], (T*)ext);
@@ -351,8 +371,6 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
     if (!out) return fail(LBWP_EINVAL, "out is NULL");
     if (!params_ok(p)) return fail(LBWP_EINVAL, "invalid lbwp_params (lattice 19|27, dtype, ncomp 1|2, sizes >= 1, tau > 0.5, struct_size)");
     if (!moments) return fail(LBWP_EINVAL, "moments is NULL");
-    if (p->scheme == LBWP_POPULATIONS && p->ncomp != 1)
-        return fail(LBWP_EUNSUPPORTED, "population-storing comparison kernel is built for ncomp == 1 only");
     const int variant = choose_variant(p);
     if (variant == 0)
         return fail(LBWP_EUNSUPPORTED, "kernel %d is not built for this combination (MARCH: D3Q27 single-component; TMA: single-component "
@@ -405,6 +423,14 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
         cudaError_t e = cudaMalloc(&c->grad, (size_t)3 * c->L.field * c->esize);
         if (e != cudaSuccess) return bail(fail(LBWP_ENOMEM, "cudaMalloc(grad): %s", cudaGetErrorString(e)));
         c->launches_per_step = 2;
+    }
+    if (p->scheme == LBWP_POPULATIONS && p->ncomp == 2) {
+        const size_t gb = (size_t)5 * c->L.field * c->esize;  // 3 gradient + 2 density fields
+        cudaError_t e = cudaMalloc(&c->grad, gb);
+        if (e != cudaSuccess) return bail(fail(LBWP_ENOMEM, "cudaMalloc(grad): %s", cudaGetErrorString(e)));
+        e = cudaMemsetAsync(c->grad, 0, gb, c->stream);
+        if (e != cudaSuccess) return bail(fail(LBWP_ECUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e)));
+        c->launches_per_step = 3;
     }
     // ghost cells and padding start defined (padding is never read by a node update)
     for (int k = 0; k < 2; ++k) {

@@ -144,4 +144,161 @@ __global__ void __launch_bounds__(256) k_pop_import(Layout L, const T* __restric
 #undef LBWP_M
 }
 
+// ---------------------------------------------------------------------------------
+// Two components ("38 populations per each fluid component"; reading C6):
+// fields [0,Q) hold the post-collision TOTAL population minus w_i, fields [Q,2Q) the
+// colour-A population (colour B = total - A).  One time step is three launches:
+//   k_pop2_density   pull, rhoA and drho of the streamed state (densities
+//                    are assessed after streaming, before the collision)
+//   k_colour_gradient (lbwp_gather.cuh) on those two fields
+//   k_pop2_step      pull, Eq. 1-2, BGK on the total, perturbation, recolouring, store
+// ---------------------------------------------------------------------------------
+template <typename T, int Q, int CX, int CY, int CZ>
+__device__ __forceinline__ void pop2_pull_a(const Layout& L, const T* __restrict__ src, long long xc, T& rhoA) {
+    constexpr int N2 = CX * CX + CY * CY + CZ * CZ;
+    if (Q == 19 && N2 == 3) return;
+    constexpr int I = dir_index<Q>(CX, CY, CZ);
+    rhoA += src[(long long)(Q + I) * L.field + xc - ((long long)CZ * L.plane + (long long)CY * L.px + CX)];
+}
+
+// dens2: two fields (rhoA, drho) in the state layout, ghosts included.
+template <typename T, int Q>
+__global__ void __launch_bounds__(256) k_pop2_density(const StepParams<T> p, T* __restrict__ dens2) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= p.L.nx || y >= p.L.ny) return;
+    const long long xc = lidx(p.L, x, y, z);
+    T f[Q];
+    Acc<T> a = {};
+    T rhoA = 0;
+#define LBWP_M(CX, CY, CZ) pop_pull<T, Q, CX, CY, CZ>(p.L, p.src, xc, f, a); pop2_pull_a<T, Q, CX, CY, CZ>(p.L, p.src, xc, rhoA);
+    LBWP_ALL_DIRS(LBWP_M)
+#undef LBWP_M
+    store_images(dens2, p.L, x, y, z, rhoA);
+    store_images(dens2 + p.L.field, p.L, x, y, z, a.rho);
+}
+
+template <typename T>
+struct Colour {
+    T Ag, nx, ny, nz, rA, kappa;  // A|G|, interface normal, rhoA/rho, beta rhoA rhoB / rho
+};
+
+template <typename T, int Q, int CX, int CY, int CZ>
+__device__ __forceinline__ void pop2_collide_store(const Layout& L, T* __restrict__ dst, int x, int y, int z,
+                                                   const T* f, const SNode<T>& eq, T omega, const Colour<T>& c) {
+    constexpr int N2 = CX * CX + CY * CY + CZ * CZ;
+    if (Q == 19 && N2 == 3) return;
+    constexpr int I = dir_index<Q>(CX, CY, CZ);
+    const T w = T(lattice_w<Q>(N2));
+    const T feq = w * bracket<T, CX, CY, CZ>(eq);
+    T h = f[I] - omega * (f[I] - feq);                                  // BGK on the total (Eq. 7)
+    const T cn = T(CX) * c.nx + T(CY) * c.ny + T(CZ) * c.nz;
+    const T Bi = N2 == 0 ? T(lattice_w<Q>(0) - 2.0 / 3.0) : w;
+    h += T(0.5) * c.Ag * (w * cn * cn - Bi);                            // perturbation (reading C6)
+    T hA = c.rA * (w + h);                                              // recolouring (reading C6)
+    if (N2 != 0) {
+        const T inorm = N2 == 1 ? T(1) : N2 == 2 ? T(0.70710678118654752440) : T(0.57735026918962576451);
+        hA += c.kappa * w * inorm * cn;
+    }
+    store_images(dst + (long long)I * L.field, L, x, y, z, h);
+    store_images(dst + (long long)(Q + I) * L.field, L, x, y, z, hA);
+}
+
+// p.grad: 3 gradient fields followed by the 2 density fields of k_pop2_density.
+template <typename T, int Q>
+__global__ void __launch_bounds__(256) k_pop2_step(const StepParams<T> p) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= p.L.nx || y >= p.L.ny) return;
+    const long long xc = lidx(p.L, x, y, z);
+    const long long F = p.L.field;
+    T f[Q];
+    Acc<T> a = {};
+#define LBWP_M(CX, CY, CZ) pop_pull<T, Q, CX, CY, CZ>(p.L, p.src, xc, f, a);
+    LBWP_ALL_DIRS(LBWP_M)
+#undef LBWP_M
+    const T rho = T(1) + a.rho;
+    const T irho = T(1) / rho;
+    const SNode<T> eq = collide_sform<T>(a.rho, a.jx * irho, a.jy * irho, a.jz * irho, T(0), T(0), T(0), T(0),
+                                         T(0), T(0), T(1));
+    const T Gx = p.grad[xc], Gy = p.grad[F + xc], Gz = p.grad[2 * F + xc];
+    const T rhoA = p.grad[3 * F + xc];
+    const T g2 = Gx * Gx + Gy * Gy + Gz * Gz;
+    const T ig = g2 > T(1e-10) ? rsqrt_t<T>(g2) : T(0);  // reading C8
+    Colour<T> c;
+    c.Ag = p.A * (g2 * ig);
+    c.nx = Gx * ig; c.ny = Gy * ig; c.nz = Gz * ig;
+    c.rA = rhoA * irho;
+    c.kappa = p.beta * c.rA * (rho - rhoA);
+#define LBWP_M(CX, CY, CZ) pop2_collide_store<T, Q, CX, CY, CZ>(p.L, p.dst, x, y, z, f, eq, p.omega, c);
+    LBWP_ALL_DIRS(LBWP_M)
+#undef LBWP_M
+}
+
+template <typename T, int Q>
+__global__ void __launch_bounds__(256) k_pop2_export(Layout L, const T* __restrict__ prev, T* __restrict__ ext) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= L.nx || y >= L.ny) return;
+    const long long xc = lidx(L, x, y, z);
+    T f[Q];
+    Acc<T> a = {};
+    T rhoA = 0;
+#define LBWP_M(CX, CY, CZ) pop_pull<T, Q, CX, CY, CZ>(L, prev, xc, f, a); pop2_pull_a<T, Q, CX, CY, CZ>(L, prev, xc, rhoA);
+    LBWP_ALL_DIRS(LBWP_M)
+#undef LBWP_M
+    const long long n = (long long)L.nx * L.ny * L.nz;
+    const long long e = ((long long)z * L.ny + y) * L.nx + x;
+    const double rho = 1.0 + (double)a.rho;
+    ext[e] = rhoA;
+    ext[n + e] = T(rho - (double)rhoA);
+    ext[2 * n + e] = T((double)a.jx / rho);
+    ext[3 * n + e] = T((double)a.jy / rho);
+    ext[4 * n + e] = T((double)a.jz / rho);
+    ext[5 * n + e] = T((double)a.pxx + 1.0 / 3.0);
+    ext[6 * n + e] = T((double)a.pyy + 1.0 / 3.0);
+    ext[7 * n + e] = T((double)a.pzz + 1.0 / 3.0);
+    ext[8 * n + e] = a.pxy;
+    ext[9 * n + e] = a.pxz;
+    ext[10 * n + e] = a.pyz;
+}
+
+template <typename T, int Q, int CX, int CY, int CZ>
+__device__ __forceinline__ void pop2_seed(const Layout& L, T* __restrict__ dst, int x, int y, int z, const SNode<T>& s, T rA) {
+    constexpr int N2 = CX * CX + CY * CY + CZ * CZ;
+    if (Q == 19 && N2 == 3) return;
+    constexpr int I = dir_index<Q>(CX, CY, CZ);
+    int tx = x - CX, ty = y - CY, tz = z - CZ;
+    tx += tx < 0 ? L.nx : 0; tx -= tx >= L.nx ? L.nx : 0;
+    ty += ty < 0 ? L.ny : 0; ty -= ty >= L.ny ? L.ny : 0;
+    tz += tz < 0 ? L.nz : 0; tz -= tz >= L.nz ? L.nz : 0;
+    const T w = T(lattice_w<Q>(N2));
+    const T h = w * bracket<T, CX, CY, CZ>(s);
+    store_images(dst + (long long)I * L.field, L, tx, ty, tz, h);
+    store_images(dst + (long long)(Q + I) * L.field, L, tx, ty, tz, rA * (w + h));  // initial split fA = rhoA/rho f
+}
+
+// ext moments (M = 11) -> Eq. 4 populations of the total, split by colour, back-shifted.
+template <typename T, int Q>
+__global__ void __launch_bounds__(256) k_pop2_import(Layout L, const T* __restrict__ ext, T* __restrict__ dst) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= L.nx || y >= L.ny) return;
+    const long long n = (long long)L.nx * L.ny * L.nz;
+    const long long e = ((long long)z * L.ny + y) * L.nx + x;
+    const double rhoA = (double)ext[e], rho = rhoA + (double)ext[n + e];
+    const SNode<T> s = collide_sform<T>(T(rho - 1.0), ext[2 * n + e], ext[3 * n + e], ext[4 * n + e],
+                                        T((double)ext[5 * n + e] - 1.0 / 3.0), T((double)ext[6 * n + e] - 1.0 / 3.0),
+                                        T((double)ext[7 * n + e] - 1.0 / 3.0), ext[8 * n + e], ext[9 * n + e],
+                                        ext[10 * n + e], T(0));
+    const T rA = T(rhoA / rho);
+#define LBWP_M(CX, CY, CZ) pop2_seed<T, Q, CX, CY, CZ>(L, dst, x, y, z, s, rA);
+    LBWP_ALL_DIRS(LBWP_M)
+#undef LBWP_M
+}
+
 }  // namespace lbwp

@@ -267,6 +267,28 @@ def test_population_kernel(lbwp, oracle, dtype, lattice):
     check(lbwp, oracle, cfg, 0, scheme="populations")
 
 
+# ---- two-component comparison kernel (one population set per colour) vs its mini-oracle:
+#      ragged box, droplet crossing the periodic boundary, tau != 1, sign(phi) ---------------------------
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("lattice", [19, 27])
+def test_population_kernel_two_component(lbwp, oracle, dtype, lattice):
+    shape = (37, 30, 33)
+    nx, ny, nz = shape
+    tg = wl.taylor_green(0, shape=shape)
+    m = wl.droplets(0, [(0.3 * nx, 0.5 * ny, 0.5 * nz), (0.95 * nx, 0.1 * ny, 0.6 * nz)], 0.25 * min(ny, nx),
+                    [0.03, -0.03], background_u=[tg[1], tg[2], tg[3]], shape=shape)
+    cfg = dict(name="pop2", moments=m, lattice=lattice, ncomp=2, tau=0.7, A=0.01, beta=0.7, dtype=dtype)
+    m0 = wl.as_dtype(m, dtype)
+    with lbwp.Lbwp(m0, lattice=lattice, dtype=dtype, ncomp=2, tau=0.7, A=0.01, beta=0.7, scheme="populations") as sim:
+        assert sim.kernel_name == "pop_pull%d_%s_c2" % (lattice, dtype)
+        assert sim.launches_per_step == 3
+    check(lbwp, oracle, cfg, 0, scheme="populations")
+    check(lbwp, oracle, cfg, 1, scheme="populations")
+    got, ref = check(lbwp, oracle, cfg, 40, scheme="populations")
+    agree = np.mean(np.sign(got[0].astype(np.float64) - got[1]) == np.sign(ref[0] - ref[1]))
+    assert agree >= 0.9999
+
+
 # ---- edge cases: degenerate boxes, zero steps, set_moments, library-owned buffers ----------
 @pytest.mark.parametrize("shape", [(1, 1, 1), (1, 7, 3), (3, 1, 33), (2, 2, 65), (5, 9, 1)])
 @pytest.mark.parametrize("kernel", ["auto", "gather"])
