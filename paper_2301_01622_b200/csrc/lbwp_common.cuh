@@ -67,21 +67,27 @@ __device__ __forceinline__ void store_images(T* __restrict__ f, const Layout& L,
     const bool by0 = (y == 0), by1 = (y == L.ny - 1);
     const bool bz0 = (z == 0), bz1 = (z == L.nz - 1);
     if (!(bx0 | bx1 | by0 | by1 | bz0 | bz1)) return;
-    // offsets of the images along each axis: 0 (the node itself) plus +n if at 0, -n if at n-1
-    long long dxs[3] = {0, 0, 0}, dys[3] = {0, 0, 0}, dzs[3] = {0, 0, 0};
-    int nxs = 1, nys = 1, nzs = 1;
-    if (bx0) dxs[nxs++] = L.nx;
-    if (bx1) dxs[nxs++] = -(long long)L.nx;
-    if (by0) dys[nys++] = (long long)L.ny * L.px;
-    if (by1) dys[nys++] = -(long long)L.ny * L.px;
-    if (bz0) dzs[nzs++] = (long long)L.nz * L.plane;
-    if (bz1) dzs[nzs++] = -(long long)L.nz * L.plane;
-    for (int k = 0; k < nzs; ++k)
-        for (int j = 0; j < nys; ++j)
-            for (int i = 0; i < nxs; ++i) {
-                if (i + j + k == 0) continue;
-                f[c + dzs[k] + dys[j] + dxs[i]] = v;
+    // image offsets along each axis: none, +n (node at 0), -n (node at n-1); a box one node thick has both.
+    // Plain selects, no indexed arrays: those would live in local memory and cost every caller stack traffic.
+    const long long xs1 = bx0 ? (long long)L.nx : 0, xs2 = bx1 ? -(long long)L.nx : 0;
+    const long long ys1 = by0 ? (long long)L.ny * L.px : 0, ys2 = by1 ? -(long long)L.ny * L.px : 0;
+    const long long zs1 = bz0 ? (long long)L.nz * L.plane : 0, zs2 = bz1 ? -(long long)L.nz * L.plane : 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const long long dz = k == 0 ? 0 : k == 1 ? zs1 : zs2;
+        if (k && !dz) continue;
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            const long long dy = j == 0 ? 0 : j == 1 ? ys1 : ys2;
+            if (j && !dy) continue;
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {
+                const long long dx = i == 0 ? 0 : i == 1 ? xs1 : xs2;
+                if ((i && !dx) || i + j + k == 0) continue;
+                f[c + dz + dy + dx] = v;
             }
+        }
+    }
 }
 
 // D3Q27 / D3Q19 weights by |c|^2 (textbook values; PAPER.md:58 leaves them to
