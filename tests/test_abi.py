@@ -48,6 +48,10 @@ def test_state_bytes_host_only(lib):
     assert lbwp.state_bytes(p2) > 11 * 8 * 256 ** 3
     pp = lbwp.make_params(lattice=19, dtype="f32", ncomp=1, shape=(64, 64, 64), tau=0.8, scheme="populations")
     assert lbwp.state_bytes(pp) > 19 * 4 * 64 ** 3
+    # two-component populations: one set per colour ("38 populations per each fluid component")
+    pp2 = lbwp.make_params(lattice=19, dtype="f32", ncomp=2, shape=(64, 64, 64), tau=1.0, A=0.01, beta=0.7,
+                           scheme="populations")
+    assert lbwp.state_bytes(pp2) == 2 * lbwp.state_bytes(pp)
 
 
 @pytest.mark.parametrize("bad", [dict(lattice=15), dict(tau=0.5), dict(tau=float("nan")), dict(ncomp=3),
