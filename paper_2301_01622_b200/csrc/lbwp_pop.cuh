@@ -207,7 +207,7 @@ __device__ __forceinline__ void pop2_collide_store(const Layout& L, T* __restric
 
 // p.grad: 3 gradient fields followed by the 2 density fields of k_pop2_density.
 template <typename T, int Q>
-__global__ void __launch_bounds__(256) k_pop2_step(const StepParams<T> p) {
+__global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 1) k_pop2_step(const StepParams<T> p) {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
     const int z = blockIdx.z;
