@@ -43,6 +43,8 @@ def _load():
         lib.lbwp_oracle_run.argtypes = run_args
         lib.lbwp_oracle_pop_run.argtypes = run_args
         lib.lbwp_oracle_threads.restype = ctypes.c_int
+        lib.lbwp_oracle_set_g2cut.argtypes = [ctypes.c_double]
+        lib.lbwp_oracle_get_g2cut.restype = ctypes.c_double
         _lib = lib
     return _lib
 
@@ -54,6 +56,14 @@ def _dp(a: np.ndarray):
 def threads() -> int:
     """OpenMP threads the step loops will use (results do not depend on it)."""
     return int(_load().lbwp_oracle_threads())
+
+
+def set_g2cut(v: float) -> float:
+    """Reading C8 threshold on |G|^2 (default 1e-10); returns the previous value.  For the pin that
+    brackets the dependence on it only: every parity run uses the default."""
+    old = float(_load().lbwp_oracle_get_g2cut())
+    _load().lbwp_oracle_set_g2cut(float(v))
+    return old
 
 
 def lattice(q: int):

@@ -16,13 +16,18 @@
  *       conservation, Taylor-Green viscosity, tau=1, lattice symmetry,
  *       independent numpy regularised-BGK-with-populations, dense brute force)
  *   two-component colour-gradient .. the operator formulas are not printed in
- *       the paper (PAPER.md:91 defers to ref. [25]); reading C6 is pinned only
- *       by what the mathematics fixes (A=0 reduction, colour mass and momentum
- *       conservation, uniform mixture, interface width, Laplace law with
- *       sigma = (2/9) A tau).  Against the paper's own code and figures:
- *       PARITY UNPINNED.
- *   population-storing BGK (comparison kernel's mini-oracle): pinned by
- *       conservation + Taylor-Green viscosity only.
+ *       the paper (PAPER.md:91 defers to ref. [25]); reading C6 is pinned by
+ *       what the mathematics fixes: A=0 reduction, colour mass and momentum
+ *       conservation, uniform mixture, Laplace law sigma = (2/9) A tau, and the
+ *       exact steady flat-interface balance phi(x+1)-phi(x) = (3 beta kappa_L/2)
+ *       [(1-phi(x)^2)+(1-phi(x+1)^2)], kappa_L = sum_i w_i c_ix^2/|c_i| (fixes
+ *       beta, the 1/|c_i| of cos(theta_i), the w_i rho factor and the sign of
+ *       the recolouring term); the |G|->0 constant of C8 is bracketed (sigma
+ *       independent of it, spurious currents not).  Against the paper's own
+ *       code and figures: PARITY UNPINNED.
+ *   population-storing BGK (comparison kernel's mini-oracle): conservation +
+ *       Taylor-Green viscosity (ncomp=1); ncomp=2: equality with the moments
+ *       run at tau=1, per-colour mass conservation, A=0 reduction to ncomp=1.
  *
  * Layout of every moment array: dense SoA [M][nz][ny][nx], x fastest.
  *   M = 10 : rho, ux, uy, uz, Pxx, Pyy, Pzz, Pxy, Pxz, Pyz          (C11, C12)
@@ -225,6 +230,15 @@ static void colour_gradient(const lattice_t *L, int nx, int ny, int nz, const do
             }
 }
 
+/* Reading C8: n = G/|G| where |G|^2 > g2cut, else n = 0 (the paper is silent on |G| -> 0).
+ * 1e-10 is the value every parity run uses; it was taken after the fp32 kernel existed (|G| <= 1e-5
+ * is below the fp32 rounding noise of phi), SURVEY proposed 1e-30.  lbwp_oracle_set_g2cut() exists
+ * only so that a pin can bracket what depends on the choice (tests/test_oracle_pins_two_component.py:
+ * the Laplace-law sigma does not, the spurious currents do). */
+static double g2cut = 1e-10;
+void lbwp_oracle_set_g2cut(double v) { g2cut = v; }
+double lbwp_oracle_get_g2cut(void) { return g2cut; }
+
 /* perturbation + recolouring of one population (shared by the moments oracle
  * and the population-storing comparison oracle: same reading C6). */
 static void colour_ops(const lattice_t *L, int i, double hp, double rhoA, double rhoB,
@@ -232,7 +246,7 @@ static void colour_ops(const lattice_t *L, int i, double hp, double rhoA, double
     const int *c = L->c[i];
     double g2 = G[0] * G[0] + G[1] * G[1] + G[2] * G[2];
     double gn = 0.0, nvec[3] = {0, 0, 0};
-    if (g2 > 1e-10) { /* C8: |G| <= 1e-5 is below the fp32 noise of phi; n := 0 */
+    if (g2 > g2cut) { /* C8 (default 1e-10: |G| <= 1e-5 is below the fp32 noise of phi); n := 0 */
         gn = sqrt(g2);
         for (int a = 0; a < 3; ++a) nvec[a] = G[a] / gn;
     }

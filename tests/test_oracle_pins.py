@@ -57,7 +57,10 @@ def test_eq8_is_bgk_of_eq4(oracle, q):
     rng = np.random.default_rng(2)
     H = np.concatenate([[1.3], rng.uniform(-0.1, 0.1, 3), rng.uniform(-1, 1, 6)])
     Heq = H.copy()
-    Heq[4:] = wl.pack1(np.array(H[0]), [np.array(v) for v in H[1:4]])[4:]
+    rho, (ux, uy, uz) = H[0], H[1:4]
+    # P^eq_ab = rho cs^2 delta_ab + rho u_a u_b (reading C2), typed out in the stored order xx,yy,zz,xy,xz,yz
+    Heq[4:] = [rho / 3 + rho * ux * ux, rho / 3 + rho * uy * uy, rho / 3 + rho * uz * uz,
+               rho * ux * uy, rho * ux * uz, rho * uy * uz]
     h, heq = oracle.reconstruct(q, H, 0.0), oracle.reconstruct(q, Heq, 0.0)
     # closed form of Eq. 5 typed out: w rho (1 + 3cu + 4.5 cu^2 - 1.5 u^2)
     c, w = oracle.lattice(q)

@@ -1,0 +1,137 @@
+"""Quantitative pins of the two-component oracle (reading C6/C8) and of the two-component population
+oracle (CPU only).  They close the holes the round-1 review found: the 1/|c_i| of cos(theta_i) in the
+recolouring term, `lbwp_oracle_pop_run(ncomp=2)`, and the dependence on the |G| -> 0 constant of C8.
+Derivations: DESIGN.md section 3 ("flat interface").
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2301_01622_b200 import workloads as wl
+
+LATTICES = [19, 27]
+
+
+def kappa_L(q):
+    """kappa_L = sum_i w_i c_ix^2 / |c_i|, typed out from the textbook weights: the two axis
+    directions along x, the eight face diagonals and (D3Q27) the eight corners with c_ix != 0."""
+    if q == 27:
+        return 2 * (2 / 27) + 8 * (1 / 54) / math.sqrt(2) + 8 * (1 / 216) / math.sqrt(3)
+    return 2 * (1 / 18) + 8 * (1 / 36) / math.sqrt(2)
+
+
+# ---- flat interface at rest, A = 0: the recolouring flux balances the lattice diffusion of colour -----------------
+# With u = 0, rho = 1, P = P^eq every total population is w_i (any tau), so reading C6 gives, for a profile that
+# depends on x only (n = +-x^),
+#     rhoA(x, t+1) = sum_i w_i rhoA(x - c_ix) + sum_i w_i (c_ix/|c_i|) K(x - c_ix),   K = beta (rhoA rhoB / rho) n_x.
+# sum_{c_ix = +-1} w_i = 1/6 and sum_{c_ix = +1} w_i/|c_i| = kappa_L/2, so a steady profile has a constant (by mirror
+# symmetry of the slab: zero) colour flux  (1/6)[rhoA(x+1) - rhoA(x)] - (kappa_L/2)[K(x+1) + K(x)] = 0, i.e. with
+# rhoA = (1 + phi)/2, rhoA rhoB = (1 - phi^2)/4:
+#     phi(x+1) - phi(x) = (3 beta kappa_L / 2) [ (1 - phi(x)^2) + (1 - phi(x+1)^2) ]        (exact, every node pair)
+# which is the trapezoidal rule of phi' = k (1 - phi^2), k = 3 beta kappa_L: phi ~ tanh(k x) (SURVEY pin P13, made
+# quantitative).  Dropping the 1/|c_i| of cos(theta_i) would give kappa_L = 1/3 instead of 0.2743 (D3Q27) / 0.2682
+# (D3Q19): 20 % off; a wrong beta, a wrong w_i rho factor or a wrong sign fail it too.
+@pytest.mark.parametrize("q", LATTICES)
+@pytest.mark.parametrize("beta", [0.5, 0.7])
+@pytest.mark.parametrize("tau", [1.0, 0.7])
+def test_flat_interface_profile(oracle, q, beta, tau):
+    n = 48
+    x = np.arange(n)
+    phi0 = np.tanh((10 - np.abs(x - n / 2 + 0.5)) / 2.0)[None, None, :] * np.ones((1, 1, n))
+    m = wl.pack2((1 + phi0) / 2, (1 - phi0) / 2, [np.zeros_like(phi0)] * 3)
+    o = oracle.run(m, lattice=q, ncomp=2, tau=tau, nsteps=3000, A=0.0, beta=beta)
+    assert np.abs(oracle.run(o, lattice=q, ncomp=2, tau=tau, nsteps=1, A=0.0, beta=beta) - o).max() < 1e-14  # steady
+    assert np.abs(o[0] + o[1] - 1).max() < 1e-12 and np.abs(o[2:5]).max() < 1e-13     # total fluid never moved
+    phi = ((o[0] - o[1]) / (o[0] + o[1]))[0, 0]
+    k = 3 * beta * kappa_L(q)
+    h = n // 2
+    left, right = phi[: h - 1], phi[1:h]                       # rising interface of the slab
+    den = (1 - left ** 2) + (1 - right ** 2)
+    sel = den > 1e-3                                           # inside the interface (n = 0 in the bulk, reading C8)
+    assert sel.sum() >= 6
+    ratio = (right - left)[sel] / den[sel]
+    assert np.abs(ratio / (k / 2) - 1).max() < 1e-9            # the exact discrete balance
+    inside = np.abs(phi[:h]) < 0.9
+    k_fit = np.polyfit(x[:h][inside], np.arctanh(phi[:h][inside]), 1)[0]
+    assert abs(k_fit / k - 1) < 0.01                           # tanh(k x), k = 3 beta kappa_L (measured: -0.2..-0.4 %)
+    assert abs(k_fit / (3 * beta / 3) - 1) > 0.15              # and NOT the profile of an un-normalised cos(theta)
+
+
+# ---- two-component population oracle (the comparison kernel's checker) ---------------------------------------------
+def _droplet_state(n=16, seed=4):
+    m = np.array(wl.config3(n)["moments"], dtype=np.float64)
+    rng = np.random.default_rng(seed)
+    m[2:5] += 0.01 * rng.uniform(-1, 1, m[2:5].shape)
+    return m
+
+
+# At tau = 1 BGK replaces every population by its equilibrium, which is what the moments-only scheme rebuilds from
+# (rho, u) when (1 - omega) = 0: the two-component population run and the two-component moments run are then the
+# same map (same perturbation, same recolouring, same streaming), to round-off.  At tau != 1 they differ
+# (the schemes "do not match exactly").
+@pytest.mark.parametrize("q", LATTICES)
+def test_population_oracle_two_component_equals_moments_at_tau_one(oracle, q):
+    m = _droplet_state()     # P = P^eq: Eq. 4 of it is the equilibrium both schemes start from
+    kw = dict(lattice=q, ncomp=2, nsteps=6, A=0.01, beta=0.7)
+    a = oracle.pop_run(m, tau=1.0, **kw)
+    b = oracle.run(m, tau=1.0, **kw)
+    assert np.abs(a - b).max() < 1e-13
+    c, d = oracle.pop_run(m, tau=0.8, **kw), oracle.run(m, tau=0.8, **kw)
+    assert 1e-6 < np.abs(c - d).max() < 1e-2
+
+
+# Each colour's mass and the total momentum are conserved by the population run too, tau != 1, A and beta on.
+@pytest.mark.parametrize("q", LATTICES)
+def test_population_oracle_two_component_conservation(oracle, q):
+    m = _droplet_state()
+    o = oracle.pop_run(m, lattice=q, ncomp=2, tau=0.7, nsteps=8, A=0.01, beta=0.7)
+    for k in (0, 1):
+        assert abs(o[k].sum() - m[k].sum()) < 1e-10
+    for a in range(3):
+        assert abs(((o[0] + o[1]) * o[2 + a]).sum() - ((m[0] + m[1]) * m[2 + a]).sum()) < 1e-11
+
+
+# A = 0: recolouring leaves the total populations alone, so the total fluid of the two-component population run is
+# the single-component population run from the total fields (any beta); with beta = 0 too, rhoA/rho is a passive
+# scalar of those populations.
+@pytest.mark.parametrize("q", LATTICES)
+@pytest.mark.parametrize("beta", [0.0, 0.7])
+def test_population_oracle_two_component_A0_reduces_to_single(oracle, q, beta):
+    m2 = _droplet_state()
+    m2[5:] += 1e-3 * np.random.default_rng(8).uniform(-1, 1, m2[5:].shape)      # off-equilibrium P
+    m1 = np.concatenate([(m2[0] + m2[1])[None], m2[2:]])
+    o2 = oracle.pop_run(m2, lattice=q, ncomp=2, tau=0.8, nsteps=6, A=0.0, beta=beta)
+    o1 = oracle.pop_run(m1, lattice=q, ncomp=1, tau=0.8, nsteps=6)
+    assert np.abs((o2[0] + o2[1]) - o1[0]).max() < 1e-13
+    assert np.abs(o2[2:] - o1[1:]).max() < 1e-13
+
+
+# ---- reading C8: the |G|^2 threshold below which n := 0 --------------------------------------------------------------
+# The paper is silent; SURVEY proposed 1e-30, the oracle (and the kernels) use 1e-10, chosen after the fp32 kernel
+# existed.  What depends on it: the surface tension does not (both terms it gates vanish with
+# |G|), the spurious currents around a static drop do (the far field keeps a direction with 1e-30).
+def test_c8_threshold_bracket(oracle):
+    n, R, steps, A, tau = 20, 6.0, 600, 0.02, 0.8
+    m = wl.droplets(n, [(n / 2, n / 2, n / 2)], R, [0.0], width=1.5)
+    res = {}
+    for cut in (1e-10, 1e-30):
+        old = oracle.set_g2cut(cut)
+        try:
+            o = oracle.run(m, lattice=27, ncomp=2, tau=tau, nsteps=steps, A=A, beta=0.7)
+        finally:
+            oracle.set_g2cut(old)
+        rho = o[0] + o[1]
+        phi = (o[0] - o[1]) / rho
+        c = n // 2
+        dp = (rho[c - 2:c + 3, c - 2:c + 3, c - 2:c + 3].mean() - rho[:3, :3, :3].mean()) / 3.0
+        r_eff = (3.0 * (phi > 0).sum() / (4.0 * math.pi)) ** (1.0 / 3.0)
+        res[cut] = (dp * r_eff / 2.0, np.abs(o[2:5]).max(), phi)
+    assert oracle.set_g2cut(1e-10) == 1e-10                                     # default restored
+    s10, s30 = res[1e-10][0], res[1e-30][0]
+    assert abs(s10 / s30 - 1) < 0.01                                            # sigma: independent of the constant
+    assert abs(s10 / (2.0 / 9.0 * A * tau) - 1) < 0.10 and abs(s30 / (2.0 / 9.0 * A * tau) - 1) < 0.10
+    assert np.array_equal(np.sign(res[1e-10][2]), np.sign(res[1e-30][2]))       # same drop
+    u10, u30 = res[1e-10][1], res[1e-30][1]
+    assert u10 < 2e-4 and u30 < 4e-4                                            # spurious currents: the part that moves
+    print(f"C8 bracket: sigma {s10:.6e} vs {s30:.6e}; max|u| {u10:.3e} (1e-10) vs {u30:.3e} (1e-30)")
