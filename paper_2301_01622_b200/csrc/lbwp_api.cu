@@ -232,15 +232,15 @@ struct TmaCtx final : lbwp_ctx {
         const dim3 b(32, 8, 1), g((X.nx + 31) / 32, (X.ny + 7) / 8, X.nz);
         steps = 0;
         cur = 0;
-        if (P.lattice == 27) lbwp::k_tma_import<T, 27><<<g, b, 0, stream>>>(X, (const T*)ext, (T*)buf[0], (T*)buf[1], T(1.0 / P.tau));
-        else lbwp::k_tma_import<T, 19><<<g, b, 0, stream>>>(X, (const T*)ext, (T*)buf[0], (T*)buf[1], T(1.0 / P.tau));
+        if (P.lattice == 27) lbwp::k_tma_import<T, 27><<<g, b, 0, stream>>>(planp->Lb[0], planp->Lb[1], (const T*)ext, (T*)buf[0], (T*)buf[1], T(1.0 / P.tau));
+        else lbwp::k_tma_import<T, 19><<<g, b, 0, stream>>>(planp->Lb[0], planp->Lb[1], (const T*)ext, (T*)buf[0], (T*)buf[1], T(1.0 / P.tau));
         CU(cudaGetLastError());
         return LBWP_OK;
     }
     int export_dense(void* ext) override {
         if (steps == 0) {
             const dim3 b(32, 8, 1), g((X.nx + 31) / 32, (X.ny + 7) / 8, X.nz);
-            lbwp::k_tma_export_raw<T><<<g, b, 0, stream>>>(X, (const T*)buf[cur ^ 1], (T*)ext);
+            lbwp::k_tma_export_raw<T><<<g, b, 0, stream>>>(planp->Lb[cur ^ 1], (const T*)buf[cur ^ 1], (T*)ext);
             CU(cudaGetLastError());
             return LBWP_OK;
         }

@@ -188,7 +188,7 @@ struct Tma2Plan final : Tma2PlanBase {
         int per_sm = 0, dev = 0, sms = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel(), C::NT + 32, C::SMEM) != cudaSuccess || per_sm < 1)
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel(), C::NT + TMA_PRODUCER_THREADS, C::SMEM) != cudaSuccess || per_sm < 1)
             per_sm = 1;
         const long long cols = (long long)(L.nx / C::TX) * (L.ny / C::TY);
         tma_choose_chunks(L.nz, cols, per_sm * sms, &lz, &gz);
@@ -207,7 +207,7 @@ struct Tma2Plan final : Tma2PlanBase {
         k_colour_collide<T, Q, ZC><<<g, b, 0, stream>>>(a);
         TmaStepParams<T> p;
         p.L = L; p.dst = (T*)raw; p.omega = T(omega); p.lz = lz;
-        kernel()<<<grid, C::NT + 32, C::SMEM, stream>>>(main_map, row_map, p);
+        kernel()<<<grid, C::NT + TMA_PRODUCER_THREADS, C::SMEM, stream>>>(main_map, row_map, p);
         return (int)cudaGetLastError();
     }
 };

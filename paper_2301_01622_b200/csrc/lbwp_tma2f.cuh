@@ -172,7 +172,7 @@ struct Tma2fPlan final : Tma2fPlanBase {
         int per_sm = 0, dev = 0, sms = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel<EPI_SFORM>(), C::NT + 32, C::SMEM) != cudaSuccess || per_sm < 1)
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel<EPI_SFORM>(), C::NT + TMA_PRODUCER_THREADS, C::SMEM) != cudaSuccess || per_sm < 1)
             per_sm = 1;
         const long long cols = (long long)(L.nx / C::TX) * (L.ny / C::TY);
         tma_choose_chunks(L.nz, cols, per_sm * sms, &lz, &gz);
@@ -184,8 +184,8 @@ struct Tma2fPlan final : Tma2fPlanBase {
     int stencil(int epi, int from, void* dst, double omega, double beta, cudaStream_t stream) const override {
         TmaStepParams<T> p;
         p.L = L; p.dst = (T*)dst; p.omega = T(omega); p.lz = lz; p.beta = T(beta);
-        if (epi == EPI_SFORM) kernel<EPI_SFORM>()<<<grid, C::NT + 32, C::SMEM, stream>>>(main_map[from], row_map[from], p);
-        else kernel<EPI_MOMENTS>()<<<grid, C::NT + 32, C::SMEM, stream>>>(main_map[from], row_map[from], p);
+        if (epi == EPI_SFORM) kernel<EPI_SFORM>()<<<grid, C::NT + TMA_PRODUCER_THREADS, C::SMEM, stream>>>(main_map[from], row_map[from], p);
+        else kernel<EPI_MOMENTS>()<<<grid, C::NT + TMA_PRODUCER_THREADS, C::SMEM, stream>>>(main_map[from], row_map[from], p);
         return (int)cudaGetLastError();
     }
 

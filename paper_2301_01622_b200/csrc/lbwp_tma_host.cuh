@@ -13,7 +13,7 @@ namespace lbwp {
 // ext: dense [10][nz][ny][nx] moments (include/lbwp.h) -> sform: XLayout S-form (x ghosts included),
 // raw: XLayout copy of the moments themselves (what lbwp_moments returns while no step was taken).
 template <typename T, int Q>
-__global__ void __launch_bounds__(256) k_tma_import(XLayout L, const T* __restrict__ ext, T* __restrict__ sform,
+__global__ void __launch_bounds__(256) k_tma_import(XLayout L, XLayout Lraw, const T* __restrict__ ext, T* __restrict__ sform,
                                                     T* __restrict__ raw, T omega) {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
@@ -21,7 +21,7 @@ __global__ void __launch_bounds__(256) k_tma_import(XLayout L, const T* __restri
     if (x >= L.nx || y >= L.ny) return;
     const long long n = (long long)L.nx * L.ny * L.nz;
     const long long e = ((long long)z * L.ny + y) * L.nx + x;
-    const long long F = L.field, c = xidx(L, x, y, z);
+    const long long F = L.field, c = xidx(Lraw, x, y, z);
     T m[10];
 #pragma unroll
     for (int f = 0; f < 10; ++f) { m[f] = ext[f * n + e]; raw[f * F + c] = m[f]; }
@@ -89,7 +89,8 @@ inline int make_state_map(CUtensorMap* out, const void* buf, const XLayout& L, i
 // One plan = one tile geometry (nodes per thread, tile x, tile y, stages; min CTAs per SM) bound to a
 // context's two buffers.  Geometry choice: the widest tile that divides the box.
 struct TmaPlanBase {
-    XLayout L;
+    XLayout L;       // layout of buffer 0
+    XLayout Lb[2];   // per buffer: the x-paired fp32 kernel keeps buffer 1 one column to the right (TmaCfg)
     int lz = 0, gz = 0, resident = 0, grid = 0;
     char tag[32] = "";
     virtual ~TmaPlanBase() {}
@@ -128,6 +129,8 @@ struct TmaPlanT final : TmaPlanBase {
 
     int setup(const XLayout& L_, void* const buf[2]) override {
         L = L_;
+        Lb[0] = Lb[1] = L;
+        if (C::PX) Lb[1].ox += 1;
         snprintf(tag, sizeof(tag), "q%d_%dx%dx%d_s%d%s", C::Q, C::TX, C::TY, C::NPT, C::NS, C::PX ? "_px" : "");
         for (int k = 0; k < 2; ++k) {
             int rc = make_state_map<T>(&main_map[k], buf[k], L, C::BW, C::TY);
@@ -142,7 +145,7 @@ struct TmaPlanT final : TmaPlanBase {
         int per_sm = 0, dev = 0, sms = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel<EPI_SFORM>(), C::NT + 32, C::SMEM) != cudaSuccess || per_sm < 1)
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel<EPI_SFORM>(), C::NT + TMA_PRODUCER_THREADS, C::SMEM) != cudaSuccess || per_sm < 1)
             per_sm = 1;
         resident = per_sm * sms;
         const long long cols = (long long)(L.nx / C::TX) * (L.ny / C::TY);
@@ -158,11 +161,12 @@ struct TmaPlanT final : TmaPlanBase {
 
     int launch(int epi, int from, void* dst, double omega, cudaStream_t stream) const override {
         TmaStepParams<T> p;
-        p.L = L; p.dst = (T*)dst; p.omega = T(omega); p.lz = lz;
+        p.L = Lb[from ^ 1]; p.dst = (T*)dst; p.omega = T(omega); p.lz = lz;   // EPI_SFORM writes the other buffer
+        p.sh = (C::PX && from == 0) ? 1 : 0;
         if (epi == EPI_SFORM)
-            kernel<EPI_SFORM>()<<<grid, C::NT + 32, C::SMEM, stream>>>(main_map[from], row_map[from], p);
+            kernel<EPI_SFORM>()<<<grid, C::NT + TMA_PRODUCER_THREADS, C::SMEM, stream>>>(main_map[from], row_map[from], p);
         else
-            kernel<EPI_MOMENTS>()<<<grid, C::NT + 32, C::SMEM, stream>>>(main_map[from], row_map[from], p);
+            kernel<EPI_MOMENTS>()<<<grid, C::NT + TMA_PRODUCER_THREADS, C::SMEM, stream>>>(main_map[from], row_map[from], p);
         return (int)cudaGetLastError();
     }
 };

@@ -10,6 +10,7 @@ namespace lbwp {
 template <typename T, int EPI, int Q = 27>
 __device__ __forceinline__ void epilogue_node(const TmaStepParams<T>& p, const T (&a)[10], int x, int y, int z) {
     const XLayout& L = p.L;
+    if (x == L.nx) x = 0;   // x-paired mode: the last pair of a row ends on node 0
     const T rho = T(1) + a[0];
     const T irho = rcp_t<T>(rho);
     const T ux = a[1] * irho, uy = a[2] * irho, uz = a[3] * irho;
@@ -52,6 +53,10 @@ __device__ __forceinline__ void epilogue_node(const TmaStepParams<T>& p, const T
 #pragma unroll
         for (int f = 0; f < 10; ++f) g[f * F] = out[f];
     }
+    if (x == 1) {                    // second right ghost column (read by the x-paired kernel from buffer 0)
+#pragma unroll
+        for (int f = 0; f < 10; ++f) d[f * F + L.nx] = out[f];
+    }
 }
 
 // The same collision over all nodes a thread owns at once (packed FMUL2/FFMA2 for the fp32 pair), and
@@ -92,20 +97,20 @@ __device__ __forceinline__ void store_sform_node(const XLayout& L, T* __restrict
     }
 }
 
-// x-paired fp32 nodes (x, x+1), x even: one 8-byte store per field; ghost images as in store_sform_node
+// x-paired fp32 nodes (x, x+1): one 8-byte store per field (the destination buffer's parity makes the pair aligned,
+// see TmaCfg).  Ghost images: writing buffer 1 (sh = 1, x odd) the last pair of a row is (nx-1, node 0), stored at
+// the columns of x = nx-1 and the ghost x = nx, and once more at the columns of the ghost x = -1 and of node 0;
+// writing buffer 0 (sh = 0, x even) the pair (0, 1) is stored once more at the ghost columns x = nx, nx+1.
 __device__ __forceinline__ void store_sform_pair(const XLayout& L, float* __restrict__ dst, const f32x2 (&out)[10], int x,
                                                  int y, int z) {
     const long long F = L.field;
     float* __restrict__ d = dst + xidx(L, x, y, z);
 #pragma unroll
     for (int f = 0; f < 10; ++f) *reinterpret_cast<float2*>(d + f * F) = make_float2(out[f].x, out[f].y);
-    if (x == 0) {
+    if (x == 0 || x + 1 == L.nx) {
+        float* __restrict__ e = x == 0 ? d + L.nx : d - L.nx;
 #pragma unroll
-        for (int f = 0; f < 10; ++f) d[f * F + L.nx] = out[f].x;
-    }
-    if (x + 2 == L.nx) {
-#pragma unroll
-        for (int f = 0; f < 10; ++f) d[f * F - L.nx + 1] = out[f].y;
+        for (int f = 0; f < 10; ++f) *reinterpret_cast<float2*>(e + f * F) = make_float2(out[f].x, out[f].y);
     }
 }
 template <typename V>
@@ -203,18 +208,27 @@ __device__ __forceinline__ TmaItem tma_item(const XLayout& L, int lz, int gx, in
 
 // CTA b handles items b, b + gridDim.x, ... (gridDim.x = number of items gives one item per CTA and
 // leaves the order to the hardware scheduler; a smaller grid makes the CTAs persistent).  Warp
-// specialisation: the last warp is the TMA producer (one elected lane), the first NW warps consume.  The
-// stage ring runs straight across item boundaries.
-// registers per thread that still let MINB CTAs of NT + 32 threads share an SM's 64 K registers
-// (warps are placed four at a time, one per scheduler, so a CTA of 17 warps is budgeted as 20)
+// specialisation: the last warpgroup is the TMA producer (one elected lane of its first warp; the other three
+// warps only take part in the register hand-over), the first NW warps consume.  The stage ring runs straight
+// across item boundaries.
+// Registers: the CTA is launched with tma_max_regs() per thread; the producer warpgroup then drops to 24 and the
+// consumers pick up what it released (setmaxnreg, SASS USETMAXREG): 96 -> 112 for 16 consumer warps.
+constexpr int TMA_PRODUCER_THREADS = 128;
+constexpr int TMA_PRODUCER_REGS = 24;
 __host__ __device__ constexpr int tma_max_regs(int threads, int minb) {
-    const int warps = (threads / 32 + 3) / 4 * 4;
-    const int r = 65536 / (minb * warps * 32) / 8 * 8;
+    const int r = 65536 / (minb * threads) / 8 * 8;
     return r > 248 ? 248 : r;
 }
+__host__ __device__ constexpr int tma_consumer_regs(int consumers, int minb) {
+    const int launch = tma_max_regs(consumers + TMA_PRODUCER_THREADS, minb);
+    const int r = (launch + (launch - TMA_PRODUCER_REGS) * TMA_PRODUCER_THREADS / consumers) / 8 * 8;
+    return r > 248 ? 248 : r;
+}
+template <int N> __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 
 template <typename T, typename C, int EPI, int MINB>
-__global__ void __maxnreg__(tma_max_regs(C::NT + 32, MINB))
+__global__ void __maxnreg__(tma_max_regs(C::NT + TMA_PRODUCER_THREADS, MINB))
 k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant__ CUtensorMap map_row,
              const TmaStepParams<T> p) {
     using S = TmaStep<T, C>;
@@ -242,7 +256,8 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
     __syncthreads();
 
     if (tid >= C::NT) {
-        // ---- producer warp: fills every free stage, up to NS planes ahead of the consumers ----
+        // ---- producer warpgroup: one lane fills every free stage, up to NS planes ahead of the consumers ----
+        setmaxnreg_dec<TMA_PRODUCER_REGS>();
         if (tid != C::NT) return;
         int ps = 0;
         uint32_t pround = 0;
@@ -254,9 +269,10 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
                 z = z < 0 ? z + L.nz : (z >= L.nz ? z - L.nz : z);          // z wraps on the load side
                 const uint32_t dst = base + (uint32_t)(ps * C::STAGE * sizeof(T));
                 mbar_expect_tx(full(ps), C::STAGE_TX_BYTES);
-                tma_load_4d(dst, &map_main, full(ps), t.x0, 0, t.y0, z);
-                tma_load_4d(dst + (uint32_t)(C::OFF_YM * sizeof(T)), &map_row, full(ps), t.x0, 0, t.ym, z);
-                tma_load_4d(dst + (uint32_t)(C::OFF_YP * sizeof(T)), &map_row, full(ps), t.x0, 0, t.yp, z);
+                const int bx = C::PX ? t.x0 + 16 / (int)sizeof(T) : t.x0 + L.ox - C::OX;   // box start column (16-byte aligned)
+                tma_load_4d(dst, &map_main, full(ps), bx, 0, t.y0, z);
+                tma_load_4d(dst + (uint32_t)(C::OFF_YM * sizeof(T)), &map_row, full(ps), bx, 0, t.ym, z);
+                tma_load_4d(dst + (uint32_t)(C::OFF_YP * sizeof(T)), &map_row, full(ps), bx, 0, t.yp, z);
                 if (++ps == C::NS) { ps = 0; ++pround; }
             }
         }
@@ -264,6 +280,7 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
     }
 
     // ---- consumer warps ----
+    setmaxnreg_inc<tma_consumer_regs(C::NT, MINB)>();
     const int tc = tid % C::COLS_T, tr = tid / C::COLS_T;
     // node n of the thread: column tx + n * DX, row tr + n * DY of the tile
     constexpr int DX = C::PX ? 1 : 0, DY = C::PX ? 0 : C::ROWS_T;
@@ -326,9 +343,9 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
 #pragma unroll
                     for (int f = 0; f < C::NA; ++f) acc[f] = P[f].get(n);
                     if (EPI == EPI_SFORM)
-                        store_state2f<T, C::Q>(L, p.dst, acc, p.omega, p.beta, ct.x0 + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
+                        store_state2f<T, C::Q>(L, p.dst, acc, p.omega, p.beta, ct.x0 + p.sh + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
                     else
-                        store_dense2<T>(L, p.dst, acc, ct.x0 + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
+                        store_dense2<T>(L, p.dst, acc, ct.x0 + p.sh + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
                 }
             } else if constexpr (C::NC == 2) {
 #pragma unroll
@@ -336,20 +353,20 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
                     T acc[C::NA];
 #pragma unroll
                     for (int f = 0; f < C::NA; ++f) acc[f] = P[f].get(n);
-                    store_raw2_node<T>(L, p.dst, acc, ct.x0 + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
+                    store_raw2_node<T>(L, p.dst, acc, ct.x0 + p.sh + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
                 }
             } else if (EPI == EPI_SFORM && kVectorEpilogue) {
                 V out[10];
                 collide_sform_v<T, V, C::NPT, C::Q>(reinterpret_cast<const V(&)[10]>(P), p.omega, out);
                 if constexpr (C::PX != 0) {
-                    store_sform_pair(L, p.dst, out, ct.x0 + tx, ct.y0 + tr, ct.z0 + i - 2);
+                    store_sform_pair(L, p.dst, out, ct.x0 + p.sh + tx, ct.y0 + tr, ct.z0 + i - 2);
                 } else {
 #pragma unroll
                     for (int n = 0; n < C::NPT; ++n) {
                         T o[10];
 #pragma unroll
                         for (int f = 0; f < 10; ++f) o[f] = out[f].get(n);
-                        store_sform_node<T>(L, p.dst, o, ct.x0 + tx, ct.y0 + tr + n * DY, ct.z0 + i - 2);
+                        store_sform_node<T>(L, p.dst, o, ct.x0 + p.sh + tx, ct.y0 + tr + n * DY, ct.z0 + i - 2);
                     }
                 }
             } else {
@@ -358,7 +375,7 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
                     T acc[10];
 #pragma unroll
                     for (int f = 0; f < 10; ++f) acc[f] = P[f].get(n);
-                    epilogue_node<T, EPI, C::Q>(p, acc, ct.x0 + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
+                    epilogue_node<T, EPI, C::Q>(p, acc, ct.x0 + p.sh + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
                 }
             }
         }

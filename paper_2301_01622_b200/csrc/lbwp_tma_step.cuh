@@ -13,6 +13,7 @@ struct TmaStepParams {
     T omega;               // 1/tau (reading C3)
     int lz;                // z planes per chunk
     T beta = T(0);         // recolouring strength (fused two-component mode only)
+    int sh = 0;            // x-paired mode: 1 if the CTA owns x0+1 .. x0+TX (source buffer of even parity), else 0
 };
 
 // Compile-time geometry of one instance.
@@ -31,8 +32,17 @@ struct TmaCfg {
     static constexpr int M = NC_ == 1 ? 10 : NC_ == 2 ? 15 : 16;   // fields per node in a stage
     static constexpr int NA = NC_ == 1 ? 10 : 11;                   // moment sums per node
     static_assert(Q_ == 27 || Q_ == 19, "lattice");
-    static constexpr int OX = 16 / (int)sizeof(T);            // halo column sits at OX-1 and OX+TX
-    static constexpr int BW = TX + 2 * OX;                    // box width: 16-byte multiple
+    // OX = shared-memory column of the first node the CTA owns (its halo columns are OX-1 and OX+TX).  The box
+    // starts at a 16-byte aligned column of the padded row (TMA faults on any other start).  Scalar modes: the box
+    // starts OX = 16 bytes left of the tile.
+    // x-paired mode: OX = 1, so that a thread's pair sits at an (odd, even) column pair and its four sources
+    // x-1 .. x+2 are two 8-byte aligned pairs: two conflict-free LDS.64 per field row.  TMA keeps the column parity
+    // of the padded global row, and the 8-byte stores of the results want the pair at (even, odd) columns of the
+    // destination, so the two ping-pong buffers differ in parity: buffer 0 keeps node x at column 4 + x, buffer 1
+    // at column 5 + x.  Reading buffer 0 the CTA owns x0+1 .. x0+TX (TmaStepParams::sh = 1), reading buffer 1 it
+    // owns x0 .. x0+TX-1 (sh = 0); in both cases the box starts at column x0 + 4.
+    static constexpr int OX = PX_ ? 1 : 16 / (int)sizeof(T);
+    static constexpr int BW = PX_ ? TX + 4 : TX + 2 * OX;     // box width: 16-byte multiple
     static constexpr int ROW = M * BW;                        // elements per tile row [field][BW]
     static constexpr int ROWS_T = PX_ ? TY : TY / NPT;        // thread rows
     static constexpr int COLS_T = PX_ ? TX / 2 : TX;          // thread columns
@@ -135,23 +145,22 @@ struct TmaStep {
         ro = xpass<V>(O[0], O[1], O[2], four);
     }
 
-    // ---- x-paired mode (C::PX): r[0][j] is the offset of node 2t in row slot j; node 2t+1 follows it ----
+    // ---- x-paired mode (C::PX): r[0][j] is the offset of node 2t in row slot j (an odd column); node 2t+1 follows ----
     // three packed pairs of field F in one source row: hi = sources (x-1, x) for cx = +1, mid = (x, x+1) for
-    // cx = 0, lo = (x+1, x+2) for cx = -1
+    // cx = 0, lo = (x+1, x+2) for cx = -1.  hi and lo are the two aligned 8-byte loads themselves.
     template <int F>
     __device__ static __forceinline__ void ld3(const T* __restrict__ s, int r0, V& hi, V& mid, V& lo) {
         const T* __restrict__ q = s + r0 + F * BW;
-        const T lm = q[-1];
-        const float2 c = *reinterpret_cast<const float2*>(q);
-        const T rp = q[2];
-        hi.x = lm; hi.y = c.x;
-        mid.x = c.x; mid.y = c.y;
-        lo.x = c.y; lo.y = rp;
+        const float2 a = *reinterpret_cast<const float2*>(q - 1);
+        const float2 b = *reinterpret_cast<const float2*>(q + 1);
+        hi.x = a.x; hi.y = a.y;
+        mid.x = a.y; mid.y = b.x;
+        lo.x = b.x; lo.y = b.y;
     }
     template <int F>
     __device__ static __forceinline__ V ldm(const T* __restrict__ s, int r0) {
-        const float2 c = *reinterpret_cast<const float2*>(s + r0 + F * BW);
-        V v; v.x = c.x; v.y = c.y;
+        const T* __restrict__ q = s + r0 + F * BW;
+        V v; v.x = q[0]; v.y = q[1];
         return v;
     }
 
