@@ -16,7 +16,7 @@
 #include "lbwp_pop.cuh"
 #include "lbwp_tma_host.cuh"
 #include "lbwp_tma2.cuh"
-#include "lbwp_tma2f.cuh"
+#include "lbwp_tma2g.cuh"
 
 namespace {
 
@@ -61,8 +61,8 @@ int state_fields(const lbwp_params* p) {
 
 bool tma_eligible(const lbwp_params* p) {
     if (p->scheme == LBWP_MOMENTS && p->ncomp == 2)
-        return p->dtype == LBWP_F32 ? lbwp::Tma2Plan<float, 27>::eligible(p->nx, p->ny)
-                                    : lbwp::Tma2Plan<double, 27>::eligible(p->nx, p->ny);
+        return p->dtype == LBWP_F32 ? lbwp::Tma2gPlan<float, 27>::eligible(p->nx, p->ny)
+                                    : lbwp::Tma2gPlan<double, 27>::eligible(p->nx, p->ny);
     if (!(p->scheme == LBWP_MOMENTS && p->ncomp == 1)) return false;
     return p->dtype == LBWP_F32 ? lbwp::tma_eligible_f32(p->nx, p->ny) : lbwp::tma_eligible_f64(p->nx, p->ny);
 }
@@ -286,25 +286,24 @@ struct Tma2Ctx final : lbwp_ctx {
     }
 };
 
-// Fused two-component TMA variant (lbwp_tma2f.cuh): two ping-pong state buffers of 16 fields.  buf[cur] = state of
-// time t; buf[cur^1] = state of time t-1 (t >= 1) or the plain moments (t = 0), which lbwp_moments needs.
+// Fused two-component TMA variant (lbwp_tma2g.cuh): two ping-pong state buffers of 11 fields, one launch per step.
+// buf[cur] = state of time t; buf[cur^1] = state of time t-1 (t >= 1) or the plain moments (t = 0), which lbwp_moments needs.
 template <typename T>
-struct Tma2fCtx final : lbwp_ctx {
-    lbwp::Tma2fPlanBase* planp = nullptr;
+struct Tma2gCtx final : lbwp_ctx {
+    lbwp::Tma2gPlanBase* planp = nullptr;
     lbwp::XLayout X;
-    ~Tma2fCtx() override { delete planp; }
+    ~Tma2gCtx() override { delete planp; }
 
     int prepare() {
-        planp = P.lattice == 27 ? (lbwp::Tma2fPlanBase*)new (std::nothrow) lbwp::Tma2fPlan<T, 27>()
-                                : (lbwp::Tma2fPlanBase*)new (std::nothrow) lbwp::Tma2fPlan<T, 19>();
+        planp = P.lattice == 27 ? (lbwp::Tma2gPlanBase*)new (std::nothrow) lbwp::Tma2gPlan<T, 27>()
+                                : (lbwp::Tma2gPlanBase*)new (std::nothrow) lbwp::Tma2gPlan<T, 19>();
         if (!planp) return fail(LBWP_ENOMEM, "no fused two-component TMA plan");
         int rc = planp->setup(X, buf);
         if (rc) return fail(rc < 0 ? LBWP_EUNSUPPORTED : LBWP_ECUDA, "fused two-component TMA plan setup failed (%d)", rc);
         return LBWP_OK;
     }
     int step_once() override {
-        int rc = planp->stencil(lbwp::EPI_SFORM, cur, buf[cur ^ 1], 1.0 / P.tau, P.beta, stream);
-        if (!rc) rc = planp->normals(buf[cur ^ 1], P.A, stream);
+        int rc = planp->stencil(lbwp::EPI_SFORM, cur, buf[cur ^ 1], 1.0 / P.tau, P.A, P.beta, stream);
         if (rc) return fail(LBWP_ECUDA, "fused two-component step launch: %s", cudaGetErrorString((cudaError_t)rc));
         cur ^= 1;
         ++steps;
@@ -313,20 +312,18 @@ struct Tma2fCtx final : lbwp_ctx {
     int import_dense(const void* ext) override {
         steps = 0;
         cur = 0;
-        int rc = planp->import_state(ext, buf[0], buf[1], 1.0 / P.tau, P.beta, stream);
+        int rc = planp->import_state(ext, buf[0], buf[1], 1.0 / P.tau, stream);
         if (rc) return fail(LBWP_ECUDA, "import launch: %s", cudaGetErrorString((cudaError_t)rc));
-        rc = planp->normals(buf[0], P.A, stream);
-        if (rc) return fail(LBWP_ECUDA, "gradient pass launch: %s", cudaGetErrorString((cudaError_t)rc));
         return LBWP_OK;
     }
     int export_dense(void* ext) override {
         if (steps == 0) {
             const dim3 b(32, 8, 1), g((X.nx + 31) / 32, (X.ny + 7) / 8, X.nz);
-            lbwp::k_tma2f_export_raw<T><<<g, b, 0, stream>>>(X, (const T*)buf[cur ^ 1], (T*)ext);
+            lbwp::k_tma2g_export_raw<T><<<g, b, 0, stream>>>(X, (const T*)buf[cur ^ 1], (T*)ext);
             CU(cudaGetLastError());
             return LBWP_OK;
         }
-        int rc = planp->stencil(lbwp::EPI_MOMENTS, cur ^ 1, ext, 1.0 / P.tau, P.beta, stream);
+        int rc = planp->stencil(lbwp::EPI_MOMENTS, cur ^ 1, ext, 1.0 / P.tau, P.A, P.beta, stream);
         if (rc) return fail(LBWP_ECUDA, "fused two-component export launch: %s", cudaGetErrorString((cudaError_t)rc));
         return LBWP_OK;
     }
@@ -359,7 +356,7 @@ size_t lbwp_state_bytes(const lbwp_params* p) {
     if (variant == 0) return 0;
     if (variant == LBWP_KERNEL_TMA) {
         const lbwp::XLayout X = lbwp::make_xlayout(p->nx, p->ny, p->nz, elem_bytes(p));
-        return (size_t)(p->ncomp == 2 ? (tma2_fused(p) ? 16 : 15) : 10) * (size_t)X.field * (size_t)elem_bytes(p);
+        return (size_t)(p->ncomp == 2 ? (tma2_fused(p) ? 11 : 15) : 10) * (size_t)X.field * (size_t)elem_bytes(p);
     }
     const lbwp::Layout L = lbwp::make_layout(p->nx, p->ny, p->nz, elem_bytes(p));
     return (size_t)state_fields(p) * (size_t)L.field * (size_t)elem_bytes(p);
@@ -388,8 +385,8 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
     if (variant == LBWP_KERNEL_TMA) {
         const lbwp::XLayout X = lbwp::make_xlayout(p->nx, p->ny, p->nz, elem_bytes(p));
         if (tma2_fused(p)) {
-            if (p->dtype == LBWP_F32) { auto* t = new (std::nothrow) Tma2fCtx<float>(); if (t) t->X = X; c = t; }
-            else { auto* t = new (std::nothrow) Tma2fCtx<double>(); if (t) t->X = X; c = t; }
+            if (p->dtype == LBWP_F32) { auto* t = new (std::nothrow) Tma2gCtx<float>(); if (t) t->X = X; c = t; }
+            else { auto* t = new (std::nothrow) Tma2gCtx<double>(); if (t) t->X = X; c = t; }
         } else if (p->ncomp == 2) {
             if (p->dtype == LBWP_F32) { auto* t = new (std::nothrow) Tma2Ctx<float>(); if (t) t->X = X; c = t; }
             else { auto* t = new (std::nothrow) Tma2Ctx<double>(); if (t) t->X = X; c = t; }
@@ -440,8 +437,8 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
     c->variant = variant;
     if (variant == LBWP_KERNEL_TMA) {
         if (tma2_fused(p)) {
-            rc = p->dtype == LBWP_F32 ? static_cast<Tma2fCtx<float>*>(c)->prepare() : static_cast<Tma2fCtx<double>*>(c)->prepare();
-            c->launches_per_step = 2;
+            rc = p->dtype == LBWP_F32 ? static_cast<Tma2gCtx<float>*>(c)->prepare() : static_cast<Tma2gCtx<double>*>(c)->prepare();
+            c->launches_per_step = 1;
         } else if (p->ncomp == 2) {
             rc = p->dtype == LBWP_F32 ? static_cast<Tma2Ctx<float>*>(c)->prepare() : static_cast<Tma2Ctx<double>*>(c)->prepare();
             c->launches_per_step = 2;

@@ -149,6 +149,16 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         if (++spins > (1u << 26)) __trap();
     }
 }
+// A consumer warp hands a stage back to the producer.  Its shared-memory READS of the stage must have returned
+// before the arrive is seen: an LDS that is still queued behind other warps' loads when the arrive goes out can be
+// overtaken by the producer's next TMA fill of the stage (seen on B200 once the scheduler had the registers to
+// issue a plane's last LDS.64 right before the arrive: about one launch in 150 at 128^3 had a few lanes read the
+// NEXT plane's values).  The fence completes every lane's outstanding loads, __syncwarp orders the lanes.
+__device__ __forceinline__ void consumer_release(uint32_t empty_bar, int tid) {
+    __threadfence_block();
+    __syncwarp();
+    if ((tid & 31) == 0) mbar_arrive(empty_bar);
+}
 // 4-D tiled load: coordinates (x, field, y, z) of the box origin
 __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2, int c3) {
     asm volatile(

@@ -1,0 +1,360 @@
+// lbwp_tma2g.cuh -- two-component colour-gradient step (reading C6), fully fused: ONE kernel per time step that reads
+// the eleven arrays of the state once and writes eleven ("22 hydro-arrays" with Flip-Flop, 163 "11
+// arrays"): 2 x 11 x sizeof = 88 B per node and step in fp32, the method's own traffic.
+//
+// State per buffer (XLayout, 11 fields, two ghost columns on each side in x):
+//   0..9  S-form of the total fluid after BGK only (Eq. 8; x 1/216, D3Q19: x 1/36), as in lbwp_tma.cuh
+//   10    rA = rhoA / rho          (rho itself is 1 + (a + (Sd_x + Sd_y + Sd_z)/3) * 216, so rhoA, rhoB follow)
+//
+// One input plane z of a work item (tile TX x TY, z chunk) passes through three phases:
+//   G  (gradient + local colour operators, once per SOURCE node of the plane, halo ring included): the phase field
+//      phi = 2 rA - 1 is differentiated on the planes z-1, z, z+1 of a halo-2 rA tile
+//      (G = 3 sum_i w_i c_i phi(x + c_i) = 6 sum_i w_i c_i rA), n = G/|G| (reading C8); the perturbation is folded
+//      into the node's S-form in place (a -= (A/2)|G|, S += (A/9)|G| n n), and the recolouring vector
+//      K = beta rhoA rhoB / rho n and the perturbation's rest population R0 = (A/3)|G| are written next to it;
+//   C  (consume2c / consume2c19 of lbwp_tma_step.cuh, unchanged): pull + projection, the linear stencil over the
+//      fifteen fields the G phase left in the stage, with the eleventh sum for colour A;
+//   E  epilogue of the plane that just completed: BGK of the new total moments (Eq. 8), rA, eleven stores.
+// This is the paper's order BGK -> perturbation -> recolouring -> streaming -> moments with the
+// BGK moved into the producer's epilogue and the two colour operators applied where the data lands in shared memory.
+//
+// Shared memory: ring of NS main stages, each TY + 2 row slots [y0-1, y0 .. y0+TY-1, y0+TY] of pitch ROWP >= 15 BW
+// (fields 0..10 arrive by TMA, one box per row; 11..14 = K, R0 from the G phase), and a ring of 5 rA planes of TY + 4
+// rows (halo 2), loaded one plane AHEAD of the main ring so that plane z+1 is resident when plane z is differentiated.
+// Both rings complete on the main stage's `full` mbarrier.
+#pragma once
+#include "lbwp_tma_host.cuh"
+
+namespace lbwp {
+
+template <typename T, typename C>
+struct Tma2gCfg {
+    static constexpr int BW = C::BW, OX = C::OX, TX = C::TX, TY = C::TY, NS = C::NS;
+    static constexpr int MT = 11;                                                   // fields that arrive by TMA
+    static constexpr int ROWP = (15 * BW * (int)sizeof(T) + 127) / 128 * 128 / (int)sizeof(T);   // row slot pitch
+    static constexpr int SLOTS = TY + 2;
+    static constexpr int STAGE = SLOTS * ROWP;                                      // elements per main stage
+    static constexpr uint32_t ROW_TX_BYTES = (uint32_t)(MT * BW * sizeof(T));
+    // rA ring: box start 32 bytes left of the tile (halo 2 in x), rows of RBW elements with 2 rows = 128-byte multiple
+    static constexpr int ROX = 32 / (int)sizeof(T);
+    static constexpr int RBW = (TX + 2 * ROX + 64 / (int)sizeof(T) - 1) / (64 / (int)sizeof(T)) * (64 / (int)sizeof(T));
+    static constexpr int RROWS = TY + 4, RNS = 5;
+    static constexpr int RPLANE = RROWS * RBW;
+    static constexpr uint32_t RPLANE_TX_BYTES = (uint32_t)(RPLANE * sizeof(T));
+    static constexpr size_t SMEM = (size_t)(NS * STAGE + RNS * RPLANE) * sizeof(T) + 2 * NS * 8 + 128;
+    static_assert((2 * RBW * sizeof(T)) % 128 == 0 && (ROWP * sizeof(T)) % 128 == 0, "TMA destinations are 128-byte aligned");
+    static_assert(ROX >= 2 && OX >= 1, "halo");
+};
+
+template <typename T>
+struct Tma2gParams {
+    XLayout L;
+    T* __restrict__ dst;   // EPI_SFORM: 11 state fields (XLayout); EPI_MOMENTS: dense external [11][nz][ny][nx]
+    T omega, A, beta;
+    int lz;
+};
+
+// finished sums (drho, j, dP_aa, P_ab, rhoA) of one node -> the eleven state fields (BGK in moment space, Eq. 8), with
+// the periodic images in the two ghost columns on each side (reading C13)
+template <typename T, int Q>
+__device__ __forceinline__ void store_state2g(const XLayout& L, T* __restrict__ dst, const T (&a)[11], T omega, int x, int y, int z) {
+    T acc[10];
+#pragma unroll
+    for (int f = 0; f < 10; ++f) acc[f] = a[f];
+    T out[11];
+    collide_sform_node<T, Q>(acc, omega, reinterpret_cast<T(&)[10]>(out));
+    out[10] = a[10] * rcp_t<T>(T(1) + a[0]);
+    const long long F = L.field;
+    T* __restrict__ d = dst + xidx(L, x, y, z);
+#pragma unroll
+    for (int f = 0; f < 11; ++f) d[f * F] = out[f];
+    if (x < 2 || x >= L.nx - 2) {
+        T* __restrict__ g = x < 2 ? d + L.nx : d - L.nx;
+#pragma unroll
+        for (int f = 0; f < 11; ++f) g[f * F] = out[f];
+    }
+}
+
+template <typename T, typename C, int EPI>
+__global__ void __maxnreg__(tma_max_regs(C::NT + TMA_PRODUCER_THREADS, 1))
+k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant__ CUtensorMap map_ra2, const __grid_constant__ CUtensorMap map_ra8,
+             const Tma2gParams<T> p) {
+    using G = Tma2gCfg<T, C>;
+    using S = TmaStep<T, C>;
+    using V = typename S::V;
+    constexpr int Q = C::Q;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const uint32_t base = (smem_u32(smem_raw) + 127u) & ~127u;
+    T* const sm = reinterpret_cast<T*>(smem_raw + (base - smem_u32(smem_raw)));
+    T* const ring = sm + G::NS * G::STAGE;
+    const uint32_t ring_u32 = base + (uint32_t)(G::NS * G::STAGE * sizeof(T));
+    const uint32_t bars = ring_u32 + (uint32_t)(G::RNS * G::RPLANE * sizeof(T));
+    auto full = [&](int s) { return bars + 8u * s; };
+    auto empty = [&](int s) { return bars + 8u * (G::NS + s); };
+
+    const XLayout& L = p.L;
+    const int tid = threadIdx.x;
+    const int gx = L.nx / C::TX, gy = L.ny / C::TY;
+    const TmaItem t = tma_item<C>(L, p.lz, gx, gy, blockIdx.x);   // one item per CTA
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < G::NS; ++s) { mbar_init(full(s), 1); mbar_init(empty(s), C::NW); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (tid >= C::NT) {
+        // ---- producer warpgroup ----
+        setmaxnreg_dec<TMA_PRODUCER_REGS>();
+        if (tid != C::NT) return;
+        auto wrapz = [&](int z) { return z < 0 ? z + L.nz : (z >= L.nz ? z - L.nz : z); };
+        auto wrapy = [&](int y) { return y < 0 ? y + L.ny : (y >= L.ny ? y - L.ny : y); };
+        const int bx = t.x0 + L.ox - C::OX, rbx = t.x0 + L.ox - G::ROX;
+        // rA plane of relative index i (plane z0 - 1 + i) -> ring slot (i + 1) % RNS
+        auto load_ra = [&](int i, uint32_t bar) {
+            const int z = wrapz(wrapz(t.z0 - 1 + i));
+            const uint32_t dst = ring_u32 + (uint32_t)(((i + 1) % G::RNS) * G::RPLANE * sizeof(T));
+            tma_load_4d(dst, &map_ra2, bar, rbx, 10, wrapy(t.y0 - 2), z);
+            tma_load_4d(dst + (uint32_t)(2 * G::RBW * sizeof(T)), &map_ra8, bar, rbx, 10, t.y0, z);
+            tma_load_4d(dst + (uint32_t)((2 + C::TY) * G::RBW * sizeof(T)), &map_ra2, bar, rbx, 10, wrapy(t.y0 + C::TY), z);
+        };
+        int ps = 0;
+        uint32_t pround = 0;
+        for (int i = 0; i < t.nin; ++i) {
+            if (pround > 0) mbar_wait(empty(ps), (pround - 1u) & 1u);
+            const int z = wrapz(t.z0 - 1 + i);
+            const uint32_t dst = base + (uint32_t)(ps * G::STAGE * sizeof(T));
+            mbar_expect_tx(full(ps), (uint32_t)G::SLOTS * G::ROW_TX_BYTES + (i == 0 ? 3u : 1u) * G::RPLANE_TX_BYTES);
+            if (i == 0) { load_ra(-1, full(ps)); load_ra(0, full(ps)); }
+            load_ra(i + 1, full(ps));
+#pragma unroll 1
+            for (int r = 0; r < G::SLOTS; ++r)
+                tma_load_4d(dst + (uint32_t)(r * G::ROWP * sizeof(T)), &map_row, full(ps), bx, 0, wrapy(t.y0 - 1 + r), z);
+            if (++ps == G::NS) { ps = 0; ++pround; }
+        }
+        return;
+    }
+
+    // ---- consumer warps ----
+    setmaxnreg_inc<tma_consumer_regs(C::NT, 1)>();
+    const int tc = tid % C::COLS_T, tr = tid / C::COLS_T;
+    constexpr int DY = C::ROWS_T;
+    int r[C::NPT][3];   // element offsets (within a stage) of the three source rows of each owned node
+#pragma unroll
+    for (int n = 0; n < C::NPT; ++n)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) r[n][j] = (tr + n * DY + j) * G::ROWP + C::OX + tc;
+
+    V a0[C::NA], a1[C::NA], a2[C::NA];
+#pragma unroll
+    for (int f = 0; f < C::NA; ++f) a0[f] = a1[f] = a2[f] = V::bc(T(0));
+
+    const T cw = Q == 27 ? T(1.0 / 216.0) : T(1.0 / 36.0);
+    const T icw = Q == 27 ? T(216) : T(36);
+    int i = 0, s = 0;
+    uint32_t par = 0;
+
+    auto plane = [&](V(&P)[C::NA], V(&Cc)[C::NA], V(&N)[C::NA]) {
+        mbar_wait(full(s), par);
+        T* const st = sm + s * G::STAGE;
+        // ---- phase G: every source node of the plane (tile + halo ring), one node per thread and pass ----
+        {
+            const T* const rm = ring + ((i + 0) % G::RNS) * G::RPLANE;   // plane z - 1  (slot of relative index i - 1)
+            const T* const rc = ring + ((i + 1) % G::RNS) * G::RPLANE;   // plane z
+            const T* const rp = ring + ((i + 2) % G::RNS) * G::RPLANE;   // plane z + 1
+            constexpr int NCOL = C::TX + 2, NNODE = NCOL * G::SLOTS;
+            for (int k = tid; k < NNODE; k += C::NT) {
+                const int row = k / NCOL, col = k - row * NCOL;        // row slot 0 .. TY+1, column 0 <-> x0 - 1
+                const int ro = (row + 1) * G::RBW + G::ROX - 1 + col;    // ring: row 0 <-> y0 - 2, column ROX <-> x0
+                T gx_ = 0, gy_ = 0, gz_ = 0;
+#pragma unroll
+                for (int cz = -1; cz <= 1; ++cz)
+#pragma unroll
+                    for (int cy = -1; cy <= 1; ++cy)
+#pragma unroll
+                        for (int cx = -1; cx <= 1; ++cx) {
+                            const int n2 = cx * cx + cy * cy + cz * cz;
+                            if (n2 == 0 || (Q == 19 && n2 == 3)) continue;
+                            const T w = T(6.0 * lattice_w<Q>(n2));
+                            const T* const pl = cz < 0 ? rm : cz == 0 ? rc : rp;
+                            const T f = pl[ro + cy * G::RBW + cx];
+                            if (cx) gx_ += T(cx) * w * f;
+                            if (cy) gy_ += T(cy) * w * f;
+                            if (cz) gz_ += T(cz) * w * f;
+                        }
+                const T g2 = gx_ * gx_ + gy_ * gy_ + gz_ * gz_;
+                const T ig = g2 > T(1e-10) ? rsqrt_t<T>(g2) : T(0);   // reading C8
+                const T g = g2 * ig;
+                const T nx = gx_ * ig, ny = gy_ * ig, nz = gz_ * ig;
+                T* const q = st + row * G::ROWP + C::OX - 1 + col;
+                const T sa = q[0], sxx = q[4 * C::BW], syy = q[5 * C::BW], szz = q[6 * C::BW];
+                const T rA = q[10 * C::BW];
+                const T rho = T(1) + icw * (sa + (sxx + syy + szz) * T(1.0 / 3.0));
+                const T Agc = cw * p.A * g;                               // c A |G|
+                q[0] = sa - Agc * T(0.5);                                 // a -= A|G| (1/3 + 1.5/9)
+                q[4 * C::BW] = sxx + T(0.5) * Agc * nx * nx;              // 4.5 (A/9)|G| n n
+                q[5 * C::BW] = syy + T(0.5) * Agc * ny * ny;
+                q[6 * C::BW] = szz + T(0.5) * Agc * nz * nz;
+                q[7 * C::BW] += Agc * nx * ny;                            // 9 (A/9)|G| n n
+                q[8 * C::BW] += Agc * nx * nz;
+                q[9 * C::BW] += Agc * ny * nz;
+                const T kap = cw * p.beta * rA * (T(1) - rA) * rho;       // c beta rhoA rhoB / rho
+                q[11 * C::BW] = kap * nx;
+                q[12 * C::BW] = kap * ny;
+                q[13 * C::BW] = kap * nz;
+                q[14 * C::BW] = p.A * g * T(1.0 / 3.0);                   // rest population (A/3)|G|
+            }
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // these writes precede the stage's next TMA fill
+        asm volatile("bar.sync 1, %0;" ::"n"(C::NT) : "memory");          // consumers only
+        // ---- phase C: pull + projection over the fifteen fields ----
+        int rs[C::NPT][3];
+#pragma unroll
+        for (int n = 0; n < C::NPT; ++n)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) rs[n][j] = r[n][j] + s * G::STAGE;
+        if constexpr (Q == 27) S::consume2c(sm, rs, P, Cc, N);
+        else S::consume2c19(sm, rs, P, Cc, N);
+        consumer_release(empty(s), tid);
+        // ---- phase E: this input plane completes output plane z0 + i - 2 ----
+        if (i >= 2) {
+#pragma unroll
+            for (int n = 0; n < C::NPT; ++n) {
+                T acc[C::NA];
+#pragma unroll
+                for (int f = 0; f < C::NA; ++f) acc[f] = P[f].get(n);
+                if (EPI == EPI_SFORM) store_state2g<T, Q>(L, p.dst, acc, p.omega, t.x0 + tc, t.y0 + tr + n * DY, t.z0 + i - 2);
+                else store_dense2<T>(L, p.dst, acc, t.x0 + tc, t.y0 + tr + n * DY, t.z0 + i - 2);
+            }
+        }
+        if (++s == G::NS) { s = 0; par ^= 1u; }
+        ++i;
+    };
+
+    while (true) {   // accumulator sets rotate with period 3
+        plane(a0, a1, a2);
+        if (i >= t.nin) break;
+        plane(a1, a2, a0);
+        if (i >= t.nin) break;
+        plane(a2, a0, a1);
+        if (i >= t.nin) break;
+    }
+}
+
+// dense external moments [11][nz][ny][nx] (rhoA, rhoB, u, P) -> the eleven state fields, and a plain copy for t = 0
+template <typename T, int Q>
+__global__ void __launch_bounds__(256) k_tma2g_import(XLayout L, const T* __restrict__ ext, T* __restrict__ state,
+                                                      T* __restrict__ raw, T omega) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= L.nx || y >= L.ny) return;
+    const long long n = (long long)L.nx * L.ny * L.nz;
+    const long long e = ((long long)z * L.ny + y) * L.nx + x;
+    const long long F = L.field, c = xidx(L, x, y, z);
+    T m[11];
+#pragma unroll
+    for (int f = 0; f < 11; ++f) { m[f] = ext[f * n + e]; raw[f * F + c] = m[f]; }
+    const double rho = (double)m[0] + (double)m[1];
+    T a[11];
+    a[0] = T(rho - 1.0);
+    for (int k = 0; k < 3; ++k) a[1 + k] = T(rho * (double)m[2 + k]);
+    for (int k = 0; k < 3; ++k) a[4 + k] = T((double)m[5 + k] - 1.0 / 3.0);
+    for (int k = 0; k < 3; ++k) a[7 + k] = m[8 + k];
+    a[10] = m[0];
+    store_state2g<T, Q>(L, state, a, omega, x, y, z);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_tma2g_export_raw(XLayout L, const T* __restrict__ raw, T* __restrict__ ext) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= L.nx || y >= L.ny) return;
+    const long long n = (long long)L.nx * L.ny * L.nz;
+    const long long e = ((long long)z * L.ny + y) * L.nx + x;
+    const long long F = L.field, c = xidx(L, x, y, z);
+#pragma unroll
+    for (int f = 0; f < 11; ++f) ext[f * n + e] = raw[f * F + c];
+}
+
+// ---- host side ---------------------------------------------------------------------------------------
+template <typename T, int Q> struct Tma2gGeom;
+template <int Q> struct Tma2gGeom<float, Q> { using C = TmaCfg<float, 2, 64, 8, 3, Q, 2>; };
+template <int Q> struct Tma2gGeom<double, Q> { using C = TmaCfg<double, 1, 32, 8, 3, Q, 2>; };
+
+struct Tma2gPlanBase {
+    virtual ~Tma2gPlanBase() {}
+    virtual int setup(const XLayout& L_, void* const buf[2]) = 0;
+    virtual int stencil(int epi, int from, void* dst, double omega, double A, double beta, cudaStream_t stream) const = 0;
+    virtual int import_state(const void* ext, void* state, void* raw, double omega, cudaStream_t stream) const = 0;
+};
+
+// tensor map over one field-major state buffer with an arbitrary box (bw, nf, rows, 1)
+template <typename T>
+inline int make_box_map(CUtensorMap* out, const void* buf, const XLayout& L, int nfields, int bw, int nf, int rows) {
+    PFN_encodeTiled enc = get_encode_tiled();
+    if (!enc) return -1;
+    const cuuint64_t dims[4] = {(cuuint64_t)L.px, (cuuint64_t)nfields, (cuuint64_t)L.ny, (cuuint64_t)L.nz};
+    const cuuint64_t strides[3] = {(cuuint64_t)L.field * sizeof(T), (cuuint64_t)L.px * sizeof(T), (cuuint64_t)L.plane * sizeof(T)};
+    const cuuint32_t box[4] = {(cuuint32_t)bw, (cuuint32_t)nf, (cuuint32_t)rows, 1};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    const CUresult r = enc(out, sizeof(T) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4,
+                           const_cast<void*>(buf), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? 0 : (int)r;
+}
+
+template <typename T, int Q>
+struct Tma2gPlan final : Tma2gPlanBase {
+    using C = typename Tma2gGeom<T, Q>::C;
+    using G = Tma2gCfg<T, C>;
+    XLayout L;
+    CUtensorMap row_map[2], ra2_map[2], ra8_map[2];
+    int lz = 0, gz = 0, grid = 0;
+
+    static bool eligible(int nx, int ny) { return nx % C::TX == 0 && ny % C::TY == 0 && nx >= 4; }
+    template <int EPI>
+    static auto kernel() { return k_step_tma2g<T, C, EPI>; }
+
+    int setup(const XLayout& L_, void* const buf[2]) override {
+        L = L_;
+        for (int k = 0; k < 2; ++k) {
+            int rc = make_box_map<T>(&row_map[k], buf[k], L, 11, C::BW, G::MT, 1);
+            if (!rc) rc = make_box_map<T>(&ra2_map[k], buf[k], L, 11, G::RBW, 1, 2);
+            if (!rc) rc = make_box_map<T>(&ra8_map[k], buf[k], L, 11, G::RBW, 1, C::TY);
+            if (rc) return rc;
+        }
+        cudaError_t e = cudaFuncSetAttribute(kernel<EPI_SFORM>(), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(kernel<EPI_MOMENTS>(), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM);
+        if (e != cudaSuccess) return (int)e;
+        int dev = 0, sms = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        const long long cols = (long long)(L.nx / C::TX) * (L.ny / C::TY);
+        tma_choose_chunks(L.nz, cols, sms, &lz, &gz);
+        grid = (int)(cols * gz);
+        return 0;
+    }
+
+    // one pass from buffer `from`: EPI_SFORM -> the eleven state fields of dst, EPI_MOMENTS -> dense moments in dst
+    int stencil(int epi, int from, void* dst, double omega, double A, double beta, cudaStream_t stream) const override {
+        Tma2gParams<T> p;
+        p.L = L; p.dst = (T*)dst; p.omega = T(omega); p.A = T(A); p.beta = T(beta); p.lz = lz;
+        if (epi == EPI_SFORM)
+            kernel<EPI_SFORM>()<<<grid, C::NT + TMA_PRODUCER_THREADS, G::SMEM, stream>>>(row_map[from], ra2_map[from], ra8_map[from], p);
+        else
+            kernel<EPI_MOMENTS>()<<<grid, C::NT + TMA_PRODUCER_THREADS, G::SMEM, stream>>>(row_map[from], ra2_map[from], ra8_map[from], p);
+        return (int)cudaGetLastError();
+    }
+
+    int import_state(const void* ext, void* state, void* raw, double omega, cudaStream_t stream) const override {
+        const dim3 b(32, 8, 1), g((L.nx + 31) / 32, (L.ny + 7) / 8, L.nz);
+        k_tma2g_import<T, Q><<<g, b, 0, stream>>>(L, (const T*)ext, (T*)state, (T*)raw, T(omega));
+        return (int)cudaGetLastError();
+    }
+};
+
+}  // namespace lbwp

@@ -100,18 +100,24 @@ struct TmaPlanBase {
     virtual int launch(int epi, int from, void* dst, double omega, cudaStream_t stream) const = 0;
 };
 
-// z chunking for a persistent grid of `ctas` CTAs over `cols` tile columns: chunks of at most LZMAX planes
-// (longer chunks let neighbouring CTAs drift apart until their shared halo rows miss L2: measured 37 -> 57
-// GLUPS at 512^3 going from 128 to 16..32 planes), minimising rounds x (planes + 2 halo planes).
+// z chunking for `ctas` resident CTAs over `cols` tile columns.  Measured rules (B200, profiles/r02_tuning.md):
+//  * several rounds of items: chunks of at most 32 planes.  Longer chunks let neighbouring CTAs drift apart until
+//    their shared halo rows miss L2 (512^3: 37 GLUPS with 128-plane chunks, 57-68 with 16-32), and every new item
+//    re-synchronises its neighbourhood;
+//  * a launch whose items all run at once (one round) marches in lock-step from the start and tolerates chunks of
+//    up to 128 planes (256^3 fp32: 2 x 64 items of 128 planes, 63.6 against 59.7 GLUPS with 9 x 64 items of 29;
+//    384 planes in one go drift apart again: 49.9 against 64.2 at 384^3), and saves the halo planes: preferred
+//    (10 % bonus) over a multi-round split of nominally equal cost.
+// Cost = rounds x (planes + 2 halo planes).
 inline void tma_choose_chunks(int nz, long long cols, int ctas, int* lz, int* gz) {
-    const int LZMAX = 32;
+    const int LZMAX = 32, LZONE = 128;
     double best = 1e300;
     for (int g = 1; g <= nz; ++g) {
         const int l = (nz + g - 1) / g;
-        if (l > LZMAX && g < nz) continue;
         if ((nz + l - 1) / l != g) continue;
         const long long rounds = (cols * g + ctas - 1) / ctas;
-        const double cost = (double)rounds * (l + 2);
+        if (l > (rounds == 1 ? LZONE : LZMAX) && g < nz) continue;
+        const double cost = (double)rounds * (l + 2) * (rounds == 1 ? 0.9 : 1.0);
         if (cost < best - 1e-9) { best = cost; *lz = l; *gz = g; }
     }
     if (const char* e = getenv("LBWP_TMA_LZ")) {   // tuning override: planes per z chunk

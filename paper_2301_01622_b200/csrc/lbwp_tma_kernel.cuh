@@ -4,63 +4,11 @@
 
 namespace lbwp {
 
-// Epilogue of one finished output node.  acc = (drho, j, dP_aa = P_aa - 1/3, P_ab), Eq. 1-3.
-//   EPI_SFORM:   BGK collision in moment space (Eq. 8), store the S-form scaled by 1/216 (D3Q19: 1/36)
-//   EPI_MOMENTS: store rho, u = j / rho (reading C11), P  (external dense layout)
-template <typename T, int EPI, int Q = 27>
-__device__ __forceinline__ void epilogue_node(const TmaStepParams<T>& p, const T (&a)[10], int x, int y, int z) {
-    const XLayout& L = p.L;
-    if (x == L.nx) x = 0;   // x-paired mode: the last pair of a row ends on node 0
-    const T rho = T(1) + a[0];
-    const T irho = rcp_t<T>(rho);
-    const T ux = a[1] * irho, uy = a[2] * irho, uz = a[3] * irho;
-    if (EPI == EPI_MOMENTS) {
-        const long long n = (long long)L.nx * L.ny * L.nz;
-        T* __restrict__ d = p.dst + ((long long)z * L.ny + y) * L.nx + x;
-        d[0] = rho;
-        d[n] = ux; d[2 * n] = uy; d[3 * n] = uz;
-        d[4 * n] = a[4] + T(1.0 / 3.0); d[5 * n] = a[5] + T(1.0 / 3.0); d[6 * n] = a[6] + T(1.0 / 3.0);
-        d[7 * n] = a[7]; d[8 * n] = a[8]; d[9 * n] = a[9];
-        return;
-    }
-    const T c = Q == 27 ? T(1.0 / 216.0) : T(1.0 / 36.0);   // common denominator of the lattice weights
-    const T om1 = T(1) - p.omega;
-    const T wx = p.omega * a[1], wy = p.omega * a[2], wz = p.omega * a[3];   // omega rho u
-    const T iso = a[0] * T(1.0 / 3.0);                                        // rho cs^2 - 1/3
-    const T sxx = fma(wx, ux, om1 * (a[4] - iso));
-    const T syy = fma(wy, uy, om1 * (a[5] - iso));
-    const T szz = fma(wz, uz, om1 * (a[6] - iso));
-    const T sxy = fma(wx, uy, om1 * a[7]);
-    const T sxz = fma(wx, uz, om1 * a[8]);
-    const T syz = fma(wy, uz, om1 * a[9]);
-    T out[10];
-    out[0] = c * fma(T(-1.5), sxx + syy + szz, a[0]);
-    out[1] = (T(3) * c) * a[1];
-    out[2] = (T(3) * c) * a[2];
-    out[3] = (T(3) * c) * a[3];
-    out[4] = (T(4.5) * c) * sxx;
-    out[5] = (T(4.5) * c) * syy;
-    out[6] = (T(4.5) * c) * szz;
-    out[7] = (T(9) * c) * sxy;
-    out[8] = (T(9) * c) * sxz;
-    out[9] = (T(9) * c) * syz;
-    const long long F = L.field;
-    T* __restrict__ d = p.dst + xidx(L, x, y, z);
-#pragma unroll
-    for (int f = 0; f < 10; ++f) d[f * F] = out[f];
-    if (x == 0 || x == L.nx - 1) {   // periodic image in the x ghost column (reading C13); nx >= 2 here
-        T* __restrict__ g = x == 0 ? d + L.nx : d - L.nx;
-#pragma unroll
-        for (int f = 0; f < 10; ++f) g[f * F] = out[f];
-    }
-    if (x == 1) {                    // second right ghost column (read by the x-paired kernel from buffer 0)
-#pragma unroll
-        for (int f = 0; f < 10; ++f) d[f * F + L.nx] = out[f];
-    }
-}
-
-// The same collision over all nodes a thread owns at once (packed FMUL2/FFMA2 for the fp32 pair), and
-// the stores of one node of the result.
+// BGK collision in moment space (Eq. 8) of the finished sums a = (drho, j, dP_aa = P_aa - 1/3, P_ab)
+// of Eq. 1-3, written as the node's S-form scaled by the common denominator of the lattice weights (1/216, D3Q19:
+// 1/36): out = c (drho - (3/2) tr S, 3 j, (9/2) S_aa, 9 S_ab), S = omega rho u u + (1 - omega)(P - rho cs^2 I).
+// The ONE implementation of the collision on the TMA path: over all nodes a thread owns at once (packed
+// FMUL2/FFMA2 for the fp32 pair) or, through collide_sform_node, for a single node.
 template <typename T, typename V, int N, int Q>
 __device__ __forceinline__ void collide_sform_v(const V (&a)[10], T omega, V (&out)[10]) {
     const T c = Q == 27 ? T(1.0 / 216.0) : T(1.0 / 36.0);
@@ -83,18 +31,55 @@ __device__ __forceinline__ void collide_sform_v(const V (&a)[10], T omega, V (&o
     out[4] = c45 * sxx; out[5] = c45 * syy; out[6] = c45 * szz;
     out[7] = c9 * sxy; out[8] = c9 * sxz; out[9] = c9 * syz;
 }
+template <typename T, int Q>
+__device__ __forceinline__ void collide_sform_node(const T (&a)[10], T omega, T (&out)[10]) {
+    Vec<T, 1> av[10], ov[10];
+#pragma unroll
+    for (int f = 0; f < 10; ++f) av[f].v = a[f];
+    collide_sform_v<T, Vec<T, 1>, 1, Q>(av, omega, ov);
+#pragma unroll
+    for (int f = 0; f < 10; ++f) out[f] = ov[f].v;
+}
 
+// stores of one node's S-form with its periodic images in the x ghost columns (reading C13; nx >= 2 here): x = -1
+// and x = nx, and x = nx + 1 (read by the x-paired kernel from buffer 0)
 template <typename T>
 __device__ __forceinline__ void store_sform_node(const XLayout& L, T* __restrict__ dst, const T (&out)[10], int x, int y, int z) {
     const long long F = L.field;
     T* __restrict__ d = dst + xidx(L, x, y, z);
 #pragma unroll
     for (int f = 0; f < 10; ++f) d[f * F] = out[f];
-    if (x == 0 || x == L.nx - 1) {   // periodic image in the x ghost column (reading C13); nx >= 2 here
+    if (x == 0 || x == L.nx - 1) {
         T* __restrict__ g = x == 0 ? d + L.nx : d - L.nx;
 #pragma unroll
         for (int f = 0; f < 10; ++f) g[f * F] = out[f];
     }
+    if (x == 1) {
+#pragma unroll
+        for (int f = 0; f < 10; ++f) d[f * F + L.nx] = out[f];
+    }
+}
+
+// Epilogue of one finished output node.  acc = (drho, j, dP_aa = P_aa - 1/3, P_ab), Eq. 1-3.
+//   EPI_SFORM:   collide (Eq. 8) and store the S-form
+//   EPI_MOMENTS: store rho, u = j / rho (reading C11), P  (external dense layout)
+template <typename T, int EPI, int Q = 27>
+__device__ __forceinline__ void epilogue_node(const TmaStepParams<T>& p, const T (&a)[10], int x, int y, int z) {
+    const XLayout& L = p.L;
+    if (x == L.nx) x = 0;   // x-paired mode: the last pair of a row ends on node 0
+    if (EPI == EPI_MOMENTS) {
+        const T irho = rcp_t<T>(T(1) + a[0]);
+        const long long n = (long long)L.nx * L.ny * L.nz;
+        T* __restrict__ d = p.dst + ((long long)z * L.ny + y) * L.nx + x;
+        d[0] = T(1) + a[0];
+        d[n] = a[1] * irho; d[2 * n] = a[2] * irho; d[3 * n] = a[3] * irho;
+        d[4 * n] = a[4] + T(1.0 / 3.0); d[5 * n] = a[5] + T(1.0 / 3.0); d[6 * n] = a[6] + T(1.0 / 3.0);
+        d[7 * n] = a[7]; d[8 * n] = a[8]; d[9 * n] = a[9];
+        return;
+    }
+    T out[10];
+    collide_sform_node<T, Q>(a, p.omega, out);
+    store_sform_node<T>(L, p.dst, out, x, y, z);
 }
 
 // x-paired fp32 nodes (x, x+1): one 8-byte store per field (the destination buffer's parity makes the pair aligned,
@@ -129,51 +114,7 @@ __device__ __forceinline__ void store_raw2_node(const XLayout& L, T* __restrict_
     d[11 * F] = (a[10] + a[10] - rho) * rcp_t<T>(rho);
 }
 
-// Fused two-component mode (C::NC == 3): finished sums (drho, j, dP_aa, P_ab, rhoA) -> the twelve state fields
-// S-form after BGK (Eq. 8, no perturbation yet), rA = rhoA/rho, kappa = beta rhoA rhoB/rho (x 1/216 or 1/36); the
-// interface fields 12..15 are written by the gradient pass (lbwp_tma2f.cuh).
-template <typename T, int Q>
-__device__ __forceinline__ void store_state2f(const XLayout& L, T* __restrict__ dst, const T (&a)[11], T omega, T beta, int x,
-                                              int y, int z) {
-    const T c = Q == 27 ? T(1.0 / 216.0) : T(1.0 / 36.0);
-    const T rho = T(1) + a[0];
-    const T irho = rcp_t<T>(rho);
-    const T ux = a[1] * irho, uy = a[2] * irho, uz = a[3] * irho;
-    const T om1 = T(1) - omega;
-    const T wx = omega * a[1], wy = omega * a[2], wz = omega * a[3];
-    const T iso = a[0] * T(1.0 / 3.0);
-    const T sxx = fma(wx, ux, om1 * (a[4] - iso));
-    const T syy = fma(wy, uy, om1 * (a[5] - iso));
-    const T szz = fma(wz, uz, om1 * (a[6] - iso));
-    const T sxy = fma(wx, uy, om1 * a[7]);
-    const T sxz = fma(wx, uz, om1 * a[8]);
-    const T syz = fma(wy, uz, om1 * a[9]);
-    T out[12];
-    out[0] = c * fma(T(-1.5), sxx + syy + szz, a[0]);
-    out[1] = (T(3) * c) * a[1];
-    out[2] = (T(3) * c) * a[2];
-    out[3] = (T(3) * c) * a[3];
-    out[4] = (T(4.5) * c) * sxx;
-    out[5] = (T(4.5) * c) * syy;
-    out[6] = (T(4.5) * c) * szz;
-    out[7] = (T(9) * c) * sxy;
-    out[8] = (T(9) * c) * sxz;
-    out[9] = (T(9) * c) * syz;
-    const T rA = a[10] * irho;
-    out[10] = rA;
-    out[11] = (c * beta) * (rA * (rho - a[10]));   // beta rhoA rhoB / rho
-    const long long F = L.field;
-    T* __restrict__ d = dst + xidx(L, x, y, z);
-#pragma unroll
-    for (int f = 0; f < 12; ++f) d[f * F] = out[f];
-    if (x == 0 || x == L.nx - 1) {
-        T* __restrict__ g = x == 0 ? d + L.nx : d - L.nx;
-#pragma unroll
-        for (int f = 0; f < 12; ++f) g[f * F] = out[f];
-    }
-}
-
-// ... and the same sums written as the external moments (rhoA, rhoB, u, P), dense [11][nz][ny][nx]
+// Two-component sums (drho, j, dP_aa, P_ab, rhoA) written as the external moments (rhoA, rhoB, u, P), dense [11][nz][ny][nx]
 template <typename T>
 __device__ __forceinline__ void store_dense2(const XLayout& L, T* __restrict__ ext, const T (&a)[11], int x, int y, int z) {
     const long long n = (long long)L.nx * L.ny * L.nz;
@@ -224,8 +165,13 @@ __host__ __device__ constexpr int tma_consumer_regs(int consumers, int minb) {
     const int r = (launch + (launch - TMA_PRODUCER_REGS) * TMA_PRODUCER_THREADS / consumers) / 8 * 8;
     return r > 248 ? 248 : r;
 }
+#ifdef LBWP_NO_SETMAXNREG
+template <int N> __device__ __forceinline__ void setmaxnreg_inc() {}
+template <int N> __device__ __forceinline__ void setmaxnreg_dec() {}
+#else
 template <int N> __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+#endif
 
 template <typename T, typename C, int EPI, int MINB>
 __global__ void __maxnreg__(tma_max_regs(C::NT + TMA_PRODUCER_THREADS, MINB))
@@ -315,39 +261,16 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
 #pragma unroll
             for (int j = 0; j < 3; ++j) rs[n][j] = r[n][j] + s * C::STAGE;
         mbar_wait(full(s), par);
-#ifdef LBWP_TMA_PROBE_NOCOMPUTE   // tuning probe only: memory-side ceiling of this access pattern
-#pragma unroll
-        for (int f = 0; f < 10; ++f) {
-#pragma unroll
-            for (int n = 0; n < C::NPT; ++n) N[f].set(n, sm[rs[n][1] + f * C::BW] + sm[rs[n][0] + f * C::BW - 1] + sm[rs[n][2] + f * C::BW + 1]);
-            P[f] = P[f] + Cc[f];
-        }
-#else
-        if constexpr (C::NC == 3 && C::Q == 27) S::consume2f(sm, rs, P, Cc, N);
-        else if constexpr (C::NC == 3) S::consume2f19(sm, rs, P, Cc, N);
-        else if constexpr (C::NC == 2 && C::Q == 27) S::consume2c(sm, rs, P, Cc, N);
+        if constexpr (C::NC == 2 && C::Q == 27) S::consume2c(sm, rs, P, Cc, N);
         else if constexpr (C::NC == 2) S::consume2c19(sm, rs, P, Cc, N);
         else if constexpr (C::Q == 27) S::consume(sm, rs, P, Cc, N);
         else S::consume19(sm, rs, P, Cc, N);
-#endif
-        __syncwarp();
-        if ((tid & 31) == 0) mbar_arrive(empty(s));
+        consumer_release(empty(s), tid);
         if (i >= 2) {                               // this input plane completes output plane z0 + i - 2
             // collision over the thread's nodes at once, except where it costs registers the stencil needs
             // (fp32 D3Q27 at 96 registers: packed epilogue spills and measured 56 vs 62 GLUPS)
             constexpr bool kVectorEpilogue = C::PX || !(C::Q == 27 && C::NPT == 2);
-            if constexpr (C::NC == 3) {
-#pragma unroll
-                for (int n = 0; n < C::NPT; ++n) {
-                    T acc[C::NA];
-#pragma unroll
-                    for (int f = 0; f < C::NA; ++f) acc[f] = P[f].get(n);
-                    if (EPI == EPI_SFORM)
-                        store_state2f<T, C::Q>(L, p.dst, acc, p.omega, p.beta, ct.x0 + p.sh + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
-                    else
-                        store_dense2<T>(L, p.dst, acc, ct.x0 + p.sh + tx + n * DX, ct.y0 + tr + n * DY, ct.z0 + i - 2);
-                }
-            } else if constexpr (C::NC == 2) {
+            if constexpr (C::NC == 2) {
 #pragma unroll
                 for (int n = 0; n < C::NPT; ++n) {
                     T acc[C::NA];

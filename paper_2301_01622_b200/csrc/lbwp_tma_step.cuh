@@ -17,9 +17,10 @@ struct TmaStepParams {
 };
 
 // Compile-time geometry of one instance.
-// NC = 1: ten S-form fields in, ten out.  NC = 2 (colour gradient, split scheme of lbwp_tma2.cuh): fifteen
-// fields in (S-form with the perturbation folded in, rhoA/rho, the recolouring vector K, the rest-population
-// term), eleven moment sums per node (rhoA added).
+// NC = 1: ten S-form fields in, ten out.  NC = 2 (colour gradient): fifteen fields per node in a stage (S-form with
+// the perturbation folded in, rhoA/rho, the recolouring vector K, the rest-population term; written by the collide
+// pass of lbwp_tma2.cuh, or in shared memory by the G phase of lbwp_tma2g.cuh), eleven moment sums per node (rhoA
+// added).
 // PX = 1 (fp32 pairs only): the thread's two nodes are x-adjacent (2t, 2t+1) instead of TY/2 rows apart: one
 // LDS.64 + two LDS.32 bring the four values a field row contributes to both nodes (instead of six LDS.32), and
 // results leave as STG.64.
@@ -27,9 +28,7 @@ template <typename T, int NPT_, int TX_, int TY_, int NS_, int Q_ = 27, int NC_ 
 struct TmaCfg {
     static constexpr int NPT = NPT_, TX = TX_, TY = TY_, NS = NS_, Q = Q_, NC = NC_, PX = PX_;
     static_assert(PX_ == 0 || (NPT_ == 2 && sizeof(T) == 4 && NC_ == 1), "x-paired mode: fp32, two nodes, one component");
-    // NC = 3: fused two-component mode (lbwp_tma2f.cuh): sixteen fields in (unperturbed S-form, rA, kappa, and
-    // the interface fields (A/2)|G|, n of the gradient pass), perturbation and recolouring applied per direction.
-    static constexpr int M = NC_ == 1 ? 10 : NC_ == 2 ? 15 : 16;   // fields per node in a stage
+    static constexpr int M = NC_ == 1 ? 10 : 15;                    // fields per node in a stage
     static constexpr int NA = NC_ == 1 ? 10 : 11;                   // moment sums per node
     static_assert(Q_ == 27 || Q_ == 19, "lattice");
     // OX = shared-memory column of the first node the CTA owns (its halo columns are OX-1 and OX+TX).  The box
@@ -216,18 +215,10 @@ struct TmaStep {
         else brackets<CY, WO_CORNERS>(s, r, E, W, O);
     }
 
-    // consume one S-form input plane z: last contribution to output plane z-1 (P), middle one to
-    // plane z (C), first one to plane z+1 (N, assigned).  Order: rho, jx, jy, jz, pxx, pyy, pzz, pxy, pxz, pyz
-    __device__ static __forceinline__ void consume(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
-                                                   V (&Cc)[C::NA], V (&N)[C::NA]) {
-        const V four = V::bc(T(4));
-        XRow<V> el, ew, eo, ml, mw_, mo_, hl, hw, ho;
-        row<-1>(s, r, four, el, ew, eo);   // sources at y+1 (cy = -1)
-        row<1>(s, r, four, hl, hw, ho);    // sources at y-1 (cy = +1)
-        row<0>(s, r, four, ml, mw_, mo_);
-        const Mom6<V> me = ypass<V>(el, ml, hl, four);
-        const Mom6<V> mw = ypass<V>(ew, mw_, hw, four);
-        const Mom6<V> mo = ypass<V>(eo, mo_, ho, four);
+    // scatter of one plane's in-plane moments into the three accumulator sets (total fluid): me = moments of the
+    // E brackets (cz = 0, already weighted), mw/mo = moments of W and O (cz = +-1)
+    __device__ static __forceinline__ void scatter27(const Mom6<V>& me, const Mom6<V>& mw, const Mom6<V>& mo, const V& four,
+                                                     V (&P)[C::NA], V (&Cc)[C::NA], V (&N)[C::NA]) {
         // cz = 0 (k = 4)
         Cc[0] = vfma(four, me.m00, Cc[0]);
         Cc[1] = vfma(four, me.m10, Cc[1]);
@@ -250,13 +241,10 @@ struct TmaStep {
     // D3Q19 (the paper's lattice): weights x 36 are 12 (rest), 2 (axis), 1 (face diagonal).
     // In-plane (cz = 0): (1,2,1) x (1,2,1) plus 8 on the centre; off-plane (cz = +-1): a plus shape,
     // 2 on the centre and 1 on the four in-plane axis neighbours.  Fields are pre-scaled by 1/36.
-    __device__ static __forceinline__ void consume19(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
-                                                     V (&Cc)[C::NA], V (&N)[C::NA]) {
+    __device__ static __forceinline__ void scatter19(const V (&El)[3], const V (&Wl)[3], const V (&Ol)[3], const V (&Em)[3],
+                                                     const V (&Wm)[3], const V (&Om)[3], const V (&Eh)[3], const V (&Wh)[3],
+                                                     const V (&Oh)[3], V (&P)[C::NA], V (&Cc)[C::NA], V (&N)[C::NA]) {
         const V two = V::bc(T(2)), eight = V::bc(T(8));
-        V El[3], Wl[3], Ol[3], Em[3], Wm[3], Om[3], Eh[3], Wh[3], Oh[3];
-        brackets_any<-1, false>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
-        brackets_any<1, false>(s, r, Eh, Wh, Oh);    // sources at y-1 (cy = +1)
-        brackets_any<0, false>(s, r, Em, Wm, Om);
         // cz = 0: separable (1,2,1) passes over E, then the extra centre weight
         const XRow<V> xl = xpass<V>(El[0], El[1], El[2], two), xm = xpass<V>(Em[0], Em[1], Em[2], two),
                       xh = xpass<V>(Eh[0], Eh[1], Eh[2], two);
@@ -277,6 +265,30 @@ struct TmaStep {
         P[0] = P[0] + n00; P[1] = P[1] + n10; P[2] = P[2] + n01; P[3] = P[3] - n00;
         P[4] = P[4] + (wx - ox); P[5] = P[5] + (wy - oy); P[6] = P[6] + n00;
         P[8] = P[8] - n10; P[9] = P[9] - n01;
+    }
+
+    // consume one S-form input plane z: last contribution to output plane z-1 (P), middle one to
+    // plane z (C), first one to plane z+1 (N, assigned).  Order: rho, jx, jy, jz, pxx, pyy, pzz, pxy, pxz, pyz
+    __device__ static __forceinline__ void consume(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
+                                                   V (&Cc)[C::NA], V (&N)[C::NA]) {
+        const V four = V::bc(T(4));
+        XRow<V> el, ew, eo, ml, mw_, mo_, hl, hw, ho;
+        row<-1>(s, r, four, el, ew, eo);   // sources at y+1 (cy = -1)
+        row<1>(s, r, four, hl, hw, ho);    // sources at y-1 (cy = +1)
+        row<0>(s, r, four, ml, mw_, mo_);
+        const Mom6<V> me = ypass<V>(el, ml, hl, four);
+        const Mom6<V> mw = ypass<V>(ew, mw_, hw, four);
+        const Mom6<V> mo = ypass<V>(eo, mo_, ho, four);
+        scatter27(me, mw, mo, four, P, Cc, N);
+    }
+
+    __device__ static __forceinline__ void consume19(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
+                                                     V (&Cc)[C::NA], V (&N)[C::NA]) {
+        V El[3], Wl[3], Ol[3], Em[3], Wm[3], Om[3], Eh[3], Wh[3], Oh[3];
+        brackets_any<-1, false>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
+        brackets_any<1, false>(s, r, Eh, Wh, Oh);    // sources at y-1 (cy = +1)
+        brackets_any<0, false>(s, r, Em, Wm, Om);
+        scatter19(El, Wl, Ol, Em, Wm, Om, Eh, Wh, Oh, P, Cc, N);
     }
 
     // Two-component plane (reading C6; fields as written by k_colour_collide in lbwp_tma2.cuh):
@@ -312,27 +324,14 @@ struct TmaStep {
         brackets<-1, true>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
         brackets<1, true>(s, r, Eh, Wh, Oh);    // sources at y-1 (cy = +1)
         brackets<0, true>(s, r, Em, Wm, Om);
-        {   // total fluid: identical to consume()
+        {   // total fluid: as in consume()
             const Mom6<V> me = ypass<V>(xpass<V>(El[0], El[1], El[2], four), xpass<V>(Em[0], Em[1], Em[2], four),
                                         xpass<V>(Eh[0], Eh[1], Eh[2], four), four);
             const Mom6<V> mw = ypass<V>(xpass<V>(Wl[0], Wl[1], Wl[2], four), xpass<V>(Wm[0], Wm[1], Wm[2], four),
                                         xpass<V>(Wh[0], Wh[1], Wh[2], four), four);
             const Mom6<V> mo = ypass<V>(xpass<V>(Ol[0], Ol[1], Ol[2], four), xpass<V>(Om[0], Om[1], Om[2], four),
                                         xpass<V>(Oh[0], Oh[1], Oh[2], four), four);
-            Cc[0] = vfma(four, me.m00, Cc[0]);
-            Cc[1] = vfma(four, me.m10, Cc[1]);
-            Cc[2] = vfma(four, me.m01, Cc[2]);
-            Cc[4] = vfma(four, me.m20, Cc[4]);
-            Cc[5] = vfma(four, me.m02, Cc[5]);
-            Cc[7] = vfma(four, me.m11, Cc[7]);
-            const V p00 = mw.m00 + mo.m00, p10 = mw.m10 + mo.m10, p01 = mw.m01 + mo.m01;
-            N[0] = p00; N[1] = p10; N[2] = p01; N[3] = p00;
-            N[4] = mw.m20 + mo.m20; N[5] = mw.m02 + mo.m02; N[6] = p00;
-            N[7] = mw.m11 + mo.m11; N[8] = p10; N[9] = p01;
-            const V n00 = mw.m00 - mo.m00, n10 = mw.m10 - mo.m10, n01 = mw.m01 - mo.m01;
-            P[0] = P[0] + n00; P[1] = P[1] + n10; P[2] = P[2] + n01; P[3] = P[3] - n00;
-            P[4] = P[4] + (mw.m20 - mo.m20); P[5] = P[5] + (mw.m02 - mo.m02); P[6] = P[6] + n00;
-            P[7] = P[7] + (mw.m11 - mo.m11); P[8] = P[8] - n10; P[9] = P[9] - n01;
+            scatter27(me, mw, mo, four, P, Cc, N);
         }
         // colour A, first part: sum_c w_c rA (1 + B_c)
         V ael, awl, aol, aem, awm, aom, aeh, awh, aoh;
@@ -383,26 +382,7 @@ struct TmaStep {
         brackets<-1, false>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
         brackets<1, false>(s, r, Eh, Wh, Oh);    // sources at y-1 (cy = +1)
         brackets<0, false>(s, r, Em, Wm, Om);
-        {   // total fluid: identical to consume19()
-            const XRow<V> xl = xpass<V>(El[0], El[1], El[2], two), xm = xpass<V>(Em[0], Em[1], Em[2], two),
-                          xh = xpass<V>(Eh[0], Eh[1], Eh[2], two);
-            Mom6<V> me = ypass<V>(xl, xm, xh, two);
-            me.m00 = vfma(eight, Em[1], me.m00);
-            Cc[0] = Cc[0] + me.m00; Cc[1] = Cc[1] + me.m10; Cc[2] = Cc[2] + me.m01;
-            Cc[4] = Cc[4] + me.m20; Cc[5] = Cc[5] + me.m02; Cc[7] = Cc[7] + me.m11;
-            const V wx = Wm[2] + Wm[0], wy = Wh[1] + Wl[1], ox = Om[2] + Om[0], oy = Oh[1] + Ol[1];
-            const V w00 = vfma(two, Wm[1], wx + wy), o00 = vfma(two, Om[1], ox + oy);
-            const V w10 = Wm[2] - Wm[0], o10 = Om[2] - Om[0];
-            const V w01 = Wh[1] - Wl[1], o01 = Oh[1] - Ol[1];
-            const V p00 = w00 + o00, p10 = w10 + o10, p01 = w01 + o01;
-            N[0] = p00; N[1] = p10; N[2] = p01; N[3] = p00;
-            N[4] = wx + ox; N[5] = wy + oy; N[6] = p00;
-            N[7] = V::bc(T(0)); N[8] = p10; N[9] = p01;
-            const V n00 = w00 - o00, n10 = w10 - o10, n01 = w01 - o01;
-            P[0] = P[0] + n00; P[1] = P[1] + n10; P[2] = P[2] + n01; P[3] = P[3] - n00;
-            P[4] = P[4] + (wx - ox); P[5] = P[5] + (wy - oy); P[6] = P[6] + n00;
-            P[8] = P[8] - n10; P[9] = P[9] - n01;
-        }
+        scatter19(El, Wl, Ol, Em, Wm, Om, Eh, Wh, Oh, P, Cc, N);   // total fluid: as in consume19()
         // colour A, first part: sum_c w_c rA (1 + B_c)
         V AEl[3], AWl[3], AOl[3], AEm[3], AWm[3], AOm[3], AEh[3], AWh[3], AOh[3];
         colour_products(s, r, 2, El, Wl, Ol, false, AEl, AWl, AOl);   // cy = -1 is row slot 2
@@ -428,212 +408,6 @@ struct TmaStep {
         const V r0 = ld<14, 0>(s, r, 1), rac = ld<10, 0>(s, r, 1);
         Cc[0] = Cc[0] + r0;
         Cc[10] = (Cc[10] + mae) + vfma(rac, r0, t0);
-        N[10] = (maw + mao) + (tin + tz);
-        P[10] = P[10] + ((maw - mao) + (tin - tz));
-    }
-
-    // ---- fused two-component mode (C::NC == 3, D3Q27) ----
-    // Fields: 0..9 S-form of the total fluid after BGK only (x 1/216), 10 rA = rhoA/rho, 11 kappa = beta rhoA rhoB/rho
-    // (x 1/216), 12 gh = (A/2)|G| (x 1/216), 13..15 n = G/|G| (0 where |G| vanishes, reading C8).
-    // Perturbation (reading C6): every direction's bracket gains gh ((c.n)^2 - 1); with e = cx nx + cy ny this is
-    //   E += gh (e^2 - 1),   W += gh (e^2 - 1) + gh nz^2,   O += 2 gh e nz      (bracket = E + cz^2 Szz + cz O),
-    // and the rest direction also gains the population (A/3)|G| = 144 gh.  Recolouring as in consume2c, K = kappa n.
-    template <int CY>
-    __device__ static __forceinline__ void colour_fold(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&E)[3], V (&W)[3],
-                                                       V (&O)[3], V (&ra)[3], V (&kx)[3], V (&ky)[3], V (&kz)[3], V& gh_mid) {
-        constexpr int J = 1 - CY;
-        const V zero = V::bc(T(0));
-#pragma unroll
-        for (int cx = -1; cx <= 1; ++cx) {
-            const int k = cx + 1;
-            V gh, nx, ny, nz, kc;
-            if (cx == -1) { ra[k] = ld<10, -1>(s, r, J); kc = ld<11, -1>(s, r, J); gh = ld<12, -1>(s, r, J);
-                            nx = ld<13, -1>(s, r, J); ny = ld<14, -1>(s, r, J); nz = ld<15, -1>(s, r, J); }
-            if (cx == 0) { ra[k] = ld<10, 0>(s, r, J); kc = ld<11, 0>(s, r, J); gh = ld<12, 0>(s, r, J);
-                           nx = ld<13, 0>(s, r, J); ny = ld<14, 0>(s, r, J); nz = ld<15, 0>(s, r, J); }
-            if (cx == 1) { ra[k] = ld<10, 1>(s, r, J); kc = ld<11, 1>(s, r, J); gh = ld<12, 1>(s, r, J);
-                           nx = ld<13, 1>(s, r, J); ny = ld<14, 1>(s, r, J); nz = ld<15, 1>(s, r, J); }
-            kx[k] = kc * nx; ky[k] = kc * ny; kz[k] = kc * nz;
-            const V gz = gh * nz;
-            const V Eg = E[k] - gh, Wg = W[k] - gh;
-            if (cx == 0 && CY == 0) {
-                E[k] = Eg;
-                W[k] = vfma(gz, nz, Wg);
-                gh_mid = gh;
-            } else {
-                V e;
-                if (cx == 0) e = CY > 0 ? ny : zero - ny;
-                else if (CY == 0) e = cx > 0 ? nx : zero - nx;
-                else if (cx > 0) e = CY > 0 ? nx + ny : nx - ny;
-                else e = CY > 0 ? ny - nx : (zero - nx) - ny;
-                const V t = gh * e;
-                E[k] = vfma(t, e, Eg);
-                W[k] = vfma(gz, nz, vfma(t, e, Wg));
-                O[k] = vfma(t + t, nz, O[k]);
-            }
-        }
-    }
-
-    // one source row of the fused two-component plane, reduced at once to what the plane sums need (keeps the
-    // live set small: the kernel runs at its register limit)
-    struct Row2f {
-        XRow<V> e, w, o;          // x-pass of the perturbed brackets
-        V ae, aw, ao;             // x-pass (zeroth moment) of rA (1 + bracket)
-        V kxd, kyc, kys, kzc, kzs;  // Kx(+1) - Kx(-1); Ky, Kz at cx = 0; their sums over cx = +-1
-    };
-    template <int CY>
-    __device__ static __forceinline__ void row2f(const T* __restrict__ s, const int (&r)[C::NPT][3], const V& four, const V& cc,
-                                                 Row2f& out, V& gh_mid) {
-        V E[3], W[3], O[3], ra[3], kx[3], ky[3], kz[3];
-        brackets<CY, true>(s, r, E, W, O);
-        colour_fold<CY>(s, r, E, W, O, ra, kx, ky, kz, gh_mid);
-        out.e = xpass<V>(E[0], E[1], E[2], four);
-        out.w = xpass<V>(W[0], W[1], W[2], four);
-        out.o = xpass<V>(O[0], O[1], O[2], four);
-        V AE[3], AW[3], AO[3];
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const V rac = ra[k] * cc;
-            AE[k] = vfma(ra[k], E[k], rac);
-            AW[k] = vfma(ra[k], W[k], rac);
-            AO[k] = ra[k] * O[k];
-        }
-        out.ae = vfma(four, AE[1], AE[2] + AE[0]);
-        out.aw = vfma(four, AW[1], AW[2] + AW[0]);
-        out.ao = vfma(four, AO[1], AO[2] + AO[0]);
-        out.kxd = kx[2] - kx[0];
-        out.kyc = ky[1]; out.kys = ky[2] + ky[0];
-        out.kzc = kz[1]; out.kzs = kz[2] + kz[0];
-    }
-
-    __device__ static __forceinline__ void consume2f(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
-                                                     V (&Cc)[C::NA], V (&N)[C::NA]) {
-        const V four = V::bc(T(4));
-        const V cc = V::bc(T(1.0 / 216.0));
-        Row2f l, m, h;
-        V ghc, ghu;
-        row2f<-1>(s, r, four, cc, l, ghu);   // sources at y+1 (cy = -1)
-        row2f<1>(s, r, four, cc, h, ghu);    // sources at y-1 (cy = +1)
-        row2f<0>(s, r, four, cc, m, ghc);
-        {   // total fluid: identical to consume()
-            const Mom6<V> me = ypass<V>(l.e, m.e, h.e, four);
-            const Mom6<V> mw = ypass<V>(l.w, m.w, h.w, four);
-            const Mom6<V> mo = ypass<V>(l.o, m.o, h.o, four);
-            Cc[0] = vfma(four, me.m00, Cc[0]);
-            Cc[1] = vfma(four, me.m10, Cc[1]);
-            Cc[2] = vfma(four, me.m01, Cc[2]);
-            Cc[4] = vfma(four, me.m20, Cc[4]);
-            Cc[5] = vfma(four, me.m02, Cc[5]);
-            Cc[7] = vfma(four, me.m11, Cc[7]);
-            const V p00 = mw.m00 + mo.m00, p10 = mw.m10 + mo.m10, p01 = mw.m01 + mo.m01;
-            N[0] = p00; N[1] = p10; N[2] = p01; N[3] = p00;
-            N[4] = mw.m20 + mo.m20; N[5] = mw.m02 + mo.m02; N[6] = p00;
-            N[7] = mw.m11 + mo.m11; N[8] = p10; N[9] = p01;
-            const V n00 = mw.m00 - mo.m00, n10 = mw.m10 - mo.m10, n01 = mw.m01 - mo.m01;
-            P[0] = P[0] + n00; P[1] = P[1] + n10; P[2] = P[2] + n01; P[3] = P[3] - n00;
-            P[4] = P[4] + (mw.m20 - mo.m20); P[5] = P[5] + (mw.m02 - mo.m02); P[6] = P[6] + n00;
-            P[7] = P[7] + (mw.m11 - mo.m11); P[8] = P[8] - n10; P[9] = P[9] - n01;
-        }
-        // colour A, first part: sum_c w_c rA (1 + B_c) with the perturbed brackets
-        const V mae = vfma(four, m.ae, h.ae + l.ae), maw = vfma(four, m.aw, h.aw + l.aw), mao = vfma(four, m.ao, h.ao + l.ao);
-        // second part: sum_{c != 0} w_c K.c / |c|; weights x 216 / |c|: 16 (axis), 4/sqrt2 (face), 1/sqrt3 (corner)
-        const V da = m.kxd + (h.kyc - l.kyc);
-        const V db = (h.kxd + l.kxd) + (h.kys - l.kys);
-        const V z1 = m.kzs + (h.kzc + l.kzc);
-        const V z2 = h.kzs + l.kzs;
-        const V f1 = V::bc(T(16)), f2 = V::bc(T(2.8284271247461903)), f3 = V::bc(T(0.57735026918962576));
-        const V t0 = vfma(f1, da, f2 * db);
-        const V tin = vfma(f2, da, f3 * db);
-        const V tz = vfma(f1, m.kzc, vfma(f2, z1, f3 * z2));
-        const V r0 = V::bc(T(144)) * ghc;   // (A/3)|G| in population units
-        Cc[0] = Cc[0] + r0;
-        // rA of the node itself: recomputed load (cheaper than keeping it live across the rows)
-        Cc[10] = vfma(four, mae, Cc[10]) + vfma(ld<10, 0>(s, r, 1), r0, t0);
-        N[10] = (maw + mao) + (tin + tz);
-        P[10] = P[10] + ((maw - mao) + (tin - tz));
-    }
-
-    // D3Q19 row of the fused two-component plane, reduced at once (cf. Row2f).  SIDES: the row cy = 0, which also
-    // carries the off-plane directions (+-1, 0, cz); rows cy = +-1 carry them at cx = 0 only.
-    struct Row2f19 {
-        XRow<V> e;                   // (1,2,1) x-pass of the perturbed E brackets
-        V e1;                        // E at cx = 0 (extra centre weight), row cy = 0 only
-        V w1, o1, ws, wd, os, od;    // W, O at cx = 0; sum / difference over cx = +-1 (row cy = 0 only)
-        V ae, ae1, aw1, ao1, aws, aos;   // the same for rA (1 + bracket)
-        V kxd, kyc, kys, kzc, kzs;
-    };
-    template <int CY>
-    __device__ static __forceinline__ void row2f19(const T* __restrict__ s, const int (&r)[C::NPT][3], const V& two, const V& cc,
-                                                   Row2f19& out, V& gh_mid) {
-        constexpr bool SIDES = CY == 0;
-        V E[3], W[3], O[3], ra[3], kx[3], ky[3], kz[3];
-        W[0] = W[2] = O[0] = O[2] = V::bc(T(0));   // no such directions on rows cy = +-1
-        brackets<CY, false>(s, r, E, W, O);
-        colour_fold<CY>(s, r, E, W, O, ra, kx, ky, kz, gh_mid);
-        out.e = xpass<V>(E[0], E[1], E[2], two);
-        V AE[3];
-#pragma unroll
-        for (int k = 0; k < 3; ++k) AE[k] = vfma(ra[k], E[k], ra[k] * cc);
-        out.ae = vfma(two, AE[1], AE[2] + AE[0]);
-        out.w1 = W[1]; out.o1 = O[1];
-        out.aw1 = vfma(ra[1], W[1], ra[1] * cc);
-        out.ao1 = ra[1] * O[1];
-        if (SIDES) {
-            out.e1 = E[1]; out.ae1 = AE[1];
-            out.ws = W[2] + W[0]; out.wd = W[2] - W[0];
-            out.os = O[2] + O[0]; out.od = O[2] - O[0];
-            out.aws = vfma(ra[2], W[2], ra[2] * cc) + vfma(ra[0], W[0], ra[0] * cc);
-            out.aos = ra[2] * O[2] + ra[0] * O[0];
-        }
-        out.kxd = kx[2] - kx[0];
-        out.kyc = ky[1]; out.kys = ky[2] + ky[0];
-        out.kzc = kz[1]; out.kzs = kz[2] + kz[0];
-    }
-
-    // Fused two-component mode on D3Q19: brackets and perturbation as above (no z-dependent parts at the in-plane
-    // corners), sums with the D3Q19 weights x 36 as in consume2c19; rest population (A/3)|G| = 24 gh.
-    __device__ static __forceinline__ void consume2f19(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
-                                                       V (&Cc)[C::NA], V (&N)[C::NA]) {
-        const V two = V::bc(T(2)), eight = V::bc(T(8));
-        const V cc = V::bc(T(1.0 / 36.0));
-        Row2f19 l, m, h;
-        V ghc, ghu;
-        row2f19<-1>(s, r, two, cc, l, ghu);
-        row2f19<1>(s, r, two, cc, h, ghu);
-        row2f19<0>(s, r, two, cc, m, ghc);
-        {   // total fluid: identical to consume19()
-            Mom6<V> me = ypass<V>(l.e, m.e, h.e, two);
-            me.m00 = vfma(eight, m.e1, me.m00);
-            Cc[0] = Cc[0] + me.m00; Cc[1] = Cc[1] + me.m10; Cc[2] = Cc[2] + me.m01;
-            Cc[4] = Cc[4] + me.m20; Cc[5] = Cc[5] + me.m02; Cc[7] = Cc[7] + me.m11;
-            const V wx = m.ws, wy = h.w1 + l.w1, ox = m.os, oy = h.o1 + l.o1;
-            const V w00 = vfma(two, m.w1, wx + wy), o00 = vfma(two, m.o1, ox + oy);
-            const V w10 = m.wd, o10 = m.od;
-            const V w01 = h.w1 - l.w1, o01 = h.o1 - l.o1;
-            const V p00 = w00 + o00, p10 = w10 + o10, p01 = w01 + o01;
-            N[0] = p00; N[1] = p10; N[2] = p01; N[3] = p00;
-            N[4] = wx + ox; N[5] = wy + oy; N[6] = p00;
-            N[7] = V::bc(T(0)); N[8] = p10; N[9] = p01;
-            const V n00 = w00 - o00, n10 = w10 - o10, n01 = w01 - o01;
-            P[0] = P[0] + n00; P[1] = P[1] + n10; P[2] = P[2] + n01; P[3] = P[3] - n00;
-            P[4] = P[4] + (wx - ox); P[5] = P[5] + (wy - oy); P[6] = P[6] + n00;
-            P[8] = P[8] - n10; P[9] = P[9] - n01;
-        }
-        // colour A, first part: sum_c w_c rA (1 + B_c) with the perturbed brackets
-        const V mae = vfma(eight, m.ae1, vfma(two, m.ae, h.ae + l.ae));
-        const V maw = vfma(two, m.aw1, m.aws + (h.aw1 + l.aw1));
-        const V mao = vfma(two, m.ao1, m.aos + (h.ao1 + l.ao1));
-        // second part: sum_{c != 0} w_c K.c / |c|; weights x 36 / |c|: 2 (axis), 1/sqrt2 (face diagonal)
-        const V da = m.kxd + (h.kyc - l.kyc);
-        const V db = (h.kxd + l.kxd) + (h.kys - l.kys);
-        const V z1 = m.kzs + (h.kzc + l.kzc);
-        const V f2 = V::bc(T(0.70710678118654752));
-        const V t0 = vfma(two, da, f2 * db);
-        const V tin = f2 * da;
-        const V tz = vfma(two, m.kzc, f2 * z1);
-        const V r0 = V::bc(T(24)) * ghc;   // (A/3)|G| in population units
-        Cc[0] = Cc[0] + r0;
-        Cc[10] = (Cc[10] + mae) + vfma(ld<10, 0>(s, r, 1), r0, t0);
         N[10] = (maw + mao) + (tin + tz);
         P[10] = P[10] + ((maw - mao) + (tin - tz));
     }

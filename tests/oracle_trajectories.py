@@ -40,13 +40,18 @@ def fp32_state_trajectory(oracle, cfg, times, m0=None):
 
 def contact_states(wl, n, radius, speed, gaps, offset_z=0.0):
     """Seeded synthetic stand-ins for the contact phase of a droplet collision at full size: the two drops of the
-    config-3/4 recipe placed on their approach line with surface gaps `gaps` (lattice units; negative = the tanh
-    interfaces overlap and a neck exists), approach speed +-`speed` along x, impact offset `offset_z`."""
+    config-3/4 recipe on their approach line with surface gaps `gaps` (lattice units; negative = the drops overlap
+    and a neck exists), approach speed +-`speed` along x, impact offset `offset_z`.  The colour field is the UNION
+    of the two tanh drops (rhoA = max of the two single-drop profiles), so that 0 <= rhoA <= 1 also where they
+    overlap (the recipe's sum would exceed 1 there)."""
     out = {}
     for g in gaps:
         d = 2.0 * radius + g                       # centre distance
         dx = np.sqrt(max(d * d - offset_z * offset_z, 0.0))
         c1 = (n / 2 - dx / 2, n / 2, n / 2 - offset_z / 2)
         c2 = (n / 2 + dx / 2, n / 2, n / 2 + offset_z / 2)
-        out[g] = wl.droplets(n, [c1, c2], radius, [speed, -speed])
+        m1 = wl.droplets(n, [c1], radius, [speed])
+        m2 = wl.droplets(n, [c2], radius, [-speed])
+        rho_a = np.maximum(m1[0], m2[0])
+        out[g] = wl.pack2(rho_a, 1.0 - rho_a, [m1[2] + m2[2], m1[3] + m2[3], m1[4] + m2[4]])
     return out
