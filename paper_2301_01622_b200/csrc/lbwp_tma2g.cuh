@@ -41,9 +41,10 @@ struct Tma2gCfg {
     static constexpr int RROWS = TY + 4, RNS = 5;
     static constexpr int RPLANE = RROWS * RBW;
     static constexpr uint32_t RPLANE_TX_BYTES = (uint32_t)(RPLANE * sizeof(T));
-    static constexpr size_t SMEM = (size_t)(NS * STAGE + RNS * RPLANE) * sizeof(T) + 2 * NS * 8 + 128;
+    static constexpr size_t SMEM = (size_t)(NS * STAGE + RNS * RPLANE) * sizeof(T) + 3 * NS * 8 + 128;
     static_assert((2 * RBW * sizeof(T)) % 128 == 0 && (ROWP * sizeof(T)) % 128 == 0, "TMA destinations are 128-byte aligned");
     static_assert(ROX >= 2 && OX >= 1, "halo");
+    static_assert(RNS >= NS + 2, "an rA plane is overwritten only after the last plane that differentiates it was consumed");
 };
 
 template <typename T>
@@ -75,14 +76,132 @@ __device__ __forceinline__ void store_state2g(const XLayout& L, T* __restrict__ 
     }
 }
 
+// ---- phase G of one unit = GN x-adjacent source nodes (fp32: a pair, all arithmetic packed; fp64: one node) ----
+// st: main stage, ring planes rm / rc / rp = rA at z-1, z, z+1; row slot 0 .. TY+1, col 0 <-> x0 - 1 (col even for GN = 2)
+template <typename T, typename C, typename G, int GN>
+__device__ __forceinline__ void colour_unit(T* __restrict__ st, const T* __restrict__ rm, const T* __restrict__ rc,
+                                            const T* __restrict__ rp, int row, int col, T A, T beta) {
+    using GV = Vec<T, GN>;
+    constexpr int Q = C::Q;
+    const int ro = (row + 1) * G::RBW + G::ROX - 1 + col;     // ring: row 0 <-> y0 - 2, column ROX <-> x0
+    // the three x taps of one ring row for the unit's nodes: m = f(x-1), c = f(x), p = f(x+1)
+    auto taps = [&](const T* __restrict__ pl, int dy, GV& m, GV& c, GV& p) {
+        const T* __restrict__ q = pl + ro + dy * G::RBW;
+        if constexpr (GN == 2) {   // ro is odd: (x-1, x) and (x+1, x+2) are the two aligned 8-byte pairs
+            const float2 a = *reinterpret_cast<const float2*>(q - 1), b = *reinterpret_cast<const float2*>(q + 1);
+            m.x = a.x; m.y = a.y; c.x = a.y; c.y = b.x; p.x = b.x; p.y = b.y;
+        } else {
+            m.v = q[-1]; c.v = q[0]; p.v = q[1];
+        }
+    };
+    GV gx, gy, gz;
+    if constexpr (Q == 27) {
+        // G = 6 sum_c w_c c rA, w_c = k(cx) k(cy) k(cz) / 216, k = (1, 4, 1): separable passes
+        const GV four = GV::bc(T(4));
+        GV X[3], Y[3], Z[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const T* __restrict__ pl = k == 0 ? rm : k == 1 ? rc : rp;
+            GV d[3], sm_[3];
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                GV m, c, p;
+                taps(pl, j - 1, m, c, p);
+                d[j] = p - m;
+                sm_[j] = vfma(four, c, p + m);
+            }
+            X[k] = vfma(four, d[1], d[2] + d[0]);
+            Y[k] = sm_[2] - sm_[0];
+            if (k != 1) Z[k] = vfma(four, sm_[1], sm_[2] + sm_[0]);
+        }
+        const GV w = GV::bc(T(6.0 / 216.0));
+        gx = w * vfma(four, X[1], X[2] + X[0]);
+        gy = w * vfma(four, Y[1], Y[2] + Y[0]);
+        gz = w * (Z[2] - Z[0]);
+    } else {
+        // D3Q19: weights x 36 = 2 (axis), 1 (face diagonal): plus-shaped sums around each axis
+        const GV two = GV::bc(T(2));
+        GV m, c, p, m0, c0, p0;
+        taps(rc, 0, m0, c0, p0);
+        GV dsum = two * (p0 - m0);                       // x: 2 d(0,0) + d(+-y, 0) + d(0, +-z)
+        GV ysum, zsum;
+        taps(rc, 1, m, c, p);  dsum = dsum + (p - m); ysum = vfma(two, c, p + m);
+        taps(rc, -1, m, c, p); dsum = dsum + (p - m); ysum = ysum - vfma(two, c, p + m);
+        taps(rp, 0, m, c, p);  dsum = dsum + (p - m); zsum = vfma(two, c, p + m);
+        taps(rm, 0, m, c, p);  dsum = dsum + (p - m); zsum = zsum - vfma(two, c, p + m);
+        taps(rp, 1, m, c, p);  ysum = ysum + c; zsum = zsum + c;
+        taps(rp, -1, m, c, p); ysum = ysum - c; zsum = zsum + c;
+        taps(rm, 1, m, c, p);  ysum = ysum + c; zsum = zsum - c;
+        taps(rm, -1, m, c, p); ysum = ysum - c; zsum = zsum - c;
+        const GV w = GV::bc(T(6.0 / 36.0));
+        gx = w * dsum; gy = w * ysum; gz = w * zsum;
+    }
+    const GV g2 = vfma(gx, gx, vfma(gy, gy, gz * gz));
+    GV ig;
+#pragma unroll
+    for (int n = 0; n < GN; ++n) ig.set(n, g2.get(n) > T(1e-10) ? rsqrt_t<T>(g2.get(n)) : T(0));   // reading C8
+    const GV g = g2 * ig, nx = gx * ig, ny = gy * ig, nz = gz * ig;
+    T* __restrict__ q = st + row * G::ROWP + C::OX - 1 + col;
+    // Away from the interface (n = 0 for every node of the warp's units, reading C8) both colour operators vanish
+    // identically: the S-form stays as it is and K = R0 = 0.  Exact, warp-uniform, and the common case.
+    bool flat = true;
+#pragma unroll
+    for (int n = 0; n < GN; ++n) flat = flat && ig.get(n) == T(0);
+    if (__all_sync(__activemask(), flat)) {
+#pragma unroll
+        for (int f = 11; f < 15; ++f)
+#pragma unroll
+            for (int n = 0; n < GN; ++n) q[f * C::BW + n] = T(0);
+        return;
+    }
+    auto ldv = [&](int f) { GV v;
+#pragma unroll
+        for (int n = 0; n < GN; ++n) v.set(n, q[f * C::BW + n]);
+        return v; };
+    auto stv = [&](int f, const GV& v) {
+#pragma unroll
+        for (int n = 0; n < GN; ++n) q[f * C::BW + n] = v.get(n); };
+    const T cw = Q == 27 ? T(1.0 / 216.0) : T(1.0 / 36.0);
+    const GV sa = ldv(0), sxx = ldv(4), syy = ldv(5), szz = ldv(6), rA = ldv(10);
+    const GV rho = vfma(GV::bc(T(1) / cw), vfma(GV::bc(T(1.0 / 3.0)), sxx + syy + szz, sa), GV::bc(T(1)));
+    const GV Agc = GV::bc(cw * A) * g, hAg = GV::bc(T(0.5)) * Agc;   // c A |G| and half of it
+    stv(0, sa - hAg);                                                  // a -= A |G| (1/3 + 1.5/9)
+    const GV hx = hAg * nx, hy = hAg * ny, hz = hAg * nz;
+    stv(4, vfma(hx, nx, sxx));                                         // Sd += 4.5 (A/9)|G| n n
+    stv(5, vfma(hy, ny, syy));
+    stv(6, vfma(hz, nz, szz));
+    const GV ax = Agc * nx;
+    stv(7, vfma(ax, ny, ldv(7)));                                      // So += 9 (A/9)|G| n n
+    stv(8, vfma(ax, nz, ldv(8)));
+    stv(9, vfma(Agc * ny, nz, ldv(9)));
+    const GV kap = GV::bc(cw * beta) * (rA * (GV::bc(T(1)) - rA)) * rho;   // c beta rhoA rhoB / rho
+    stv(11, kap * nx);
+    stv(12, kap * ny);
+    stv(13, kap * nz);
+    stv(14, GV::bc(A * T(1.0 / 3.0)) * g);                              // rest population (A/3)|G|
+}
+
+// Thread roles: warps [0, NW) consume (phase C + E), the next warpgroup differentiates (phase G), the last warpgroup
+// produces (one lane issues the TMA loads).  Barriers per stage: full (TMA landed) -> gdone (phase G finished) ->
+// empty (phase C finished).  Registers are handed from the producer and G warpgroups to the consumers (setmaxnreg).
+constexpr int TMA2G_G_THREADS = 128, TMA2G_G_REGS = 80;
+__host__ __device__ constexpr int tma2g_threads(int consumers) { return consumers + TMA2G_G_THREADS + TMA_PRODUCER_THREADS; }
+__host__ __device__ constexpr int tma2g_consumer_regs(int consumers) {
+    const int launch = tma_max_regs(tma2g_threads(consumers), 1);
+    const int r = (launch * tma2g_threads(consumers) - TMA_PRODUCER_THREADS * TMA_PRODUCER_REGS - TMA2G_G_THREADS * TMA2G_G_REGS) / consumers / 8 * 8;
+    return r > 248 ? 248 : r;
+}
+
 template <typename T, typename C, int EPI>
-__global__ void __maxnreg__(tma_max_regs(C::NT + TMA_PRODUCER_THREADS, 1))
+__global__ void __maxnreg__(tma_max_regs(tma2g_threads(C::NT), 1))
 k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant__ CUtensorMap map_ra2, const __grid_constant__ CUtensorMap map_ra8,
              const Tma2gParams<T> p) {
     using G = Tma2gCfg<T, C>;
     using S = TmaStep<T, C>;
     using V = typename S::V;
     constexpr int Q = C::Q;
+    constexpr int GN = sizeof(T) == 4 ? 2 : 1;
+    static_assert(tma_max_regs(tma2g_threads(C::NT), 1) >= TMA2G_G_REGS, "the G warpgroup only ever releases registers");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 127u) & ~127u;
     T* const sm = reinterpret_cast<T*>(smem_raw + (base - smem_u32(smem_raw)));
@@ -91,6 +210,7 @@ k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant_
     const uint32_t bars = ring_u32 + (uint32_t)(G::RNS * G::RPLANE * sizeof(T));
     auto full = [&](int s) { return bars + 8u * s; };
     auto empty = [&](int s) { return bars + 8u * (G::NS + s); };
+    auto gdone = [&](int s) { return bars + 8u * (2 * G::NS + s); };
 
     const XLayout& L = p.L;
     const int tid = threadIdx.x;
@@ -99,15 +219,15 @@ k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant_
 
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < G::NS; ++s) { mbar_init(full(s), 1); mbar_init(empty(s), C::NW); }
+        for (int s = 0; s < G::NS; ++s) { mbar_init(full(s), 1); mbar_init(empty(s), C::NW); mbar_init(gdone(s), TMA2G_G_THREADS / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    if (tid >= C::NT) {
+    if (tid >= C::NT + TMA2G_G_THREADS) {
         // ---- producer warpgroup ----
         setmaxnreg_dec<TMA_PRODUCER_REGS>();
-        if (tid != C::NT) return;
+        if (tid != C::NT + TMA2G_G_THREADS) return;
         auto wrapz = [&](int z) { return z < 0 ? z + L.nz : (z >= L.nz ? z - L.nz : z); };
         auto wrapy = [&](int y) { return y < 0 ? y + L.ny : (y >= L.ny ? y - L.ny : y); };
         const int bx = t.x0 + L.ox - C::OX, rbx = t.x0 + L.ox - G::ROX;
@@ -136,8 +256,34 @@ k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant_
         return;
     }
 
-    // ---- consumer warps ----
-    setmaxnreg_inc<tma_consumer_regs(C::NT, 1)>();
+    if (tid >= C::NT) {
+        // ---- phase G warpgroup: every source node of each plane (tile + halo ring) ----
+        setmaxnreg_dec<TMA2G_G_REGS>();
+        const int gt = tid - C::NT;
+        constexpr int NU = (C::TX + 2) / GN, NUNITS = NU * G::SLOTS;
+        static_assert((C::TX + 2) % GN == 0, "units tile the source row");
+        int s = 0;
+        uint32_t par = 0;
+        for (int i = 0; i < t.nin; ++i) {
+            mbar_wait(full(s), par);
+            T* const st = sm + s * G::STAGE;
+            const T* const rm = ring + ((i + 0) % G::RNS) * G::RPLANE;   // plane z - 1 (relative index i - 1)
+            const T* const rc = ring + ((i + 1) % G::RNS) * G::RPLANE;   // plane z
+            const T* const rp = ring + ((i + 2) % G::RNS) * G::RPLANE;   // plane z + 1
+#pragma unroll 1
+            for (int u = gt; u < NUNITS; u += TMA2G_G_THREADS) {
+                const int row = u / NU;
+                colour_unit<T, C, G, GN>(st, rm, rc, rp, row, (u - row * NU) * GN, p.A, p.beta);
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // these writes precede the stage's next TMA fill
+            consumer_release(gdone(s), tid);
+            if (++s == G::NS) { s = 0; par ^= 1u; }
+        }
+        return;
+    }
+
+    // ---- consumer warps: phases C and E ----
+    setmaxnreg_inc<tma2g_consumer_regs(C::NT)>();
     const int tc = tid % C::COLS_T, tr = tid / C::COLS_T;
     constexpr int DY = C::ROWS_T;
     int r[C::NPT][3];   // element offsets (within a stage) of the three source rows of each owned node
@@ -150,64 +296,11 @@ k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant_
 #pragma unroll
     for (int f = 0; f < C::NA; ++f) a0[f] = a1[f] = a2[f] = V::bc(T(0));
 
-    const T cw = Q == 27 ? T(1.0 / 216.0) : T(1.0 / 36.0);
-    const T icw = Q == 27 ? T(216) : T(36);
     int i = 0, s = 0;
     uint32_t par = 0;
 
     auto plane = [&](V(&P)[C::NA], V(&Cc)[C::NA], V(&N)[C::NA]) {
-        mbar_wait(full(s), par);
-        T* const st = sm + s * G::STAGE;
-        // ---- phase G: every source node of the plane (tile + halo ring), one node per thread and pass ----
-        {
-            const T* const rm = ring + ((i + 0) % G::RNS) * G::RPLANE;   // plane z - 1  (slot of relative index i - 1)
-            const T* const rc = ring + ((i + 1) % G::RNS) * G::RPLANE;   // plane z
-            const T* const rp = ring + ((i + 2) % G::RNS) * G::RPLANE;   // plane z + 1
-            constexpr int NCOL = C::TX + 2, NNODE = NCOL * G::SLOTS;
-            for (int k = tid; k < NNODE; k += C::NT) {
-                const int row = k / NCOL, col = k - row * NCOL;        // row slot 0 .. TY+1, column 0 <-> x0 - 1
-                const int ro = (row + 1) * G::RBW + G::ROX - 1 + col;    // ring: row 0 <-> y0 - 2, column ROX <-> x0
-                T gx_ = 0, gy_ = 0, gz_ = 0;
-#pragma unroll
-                for (int cz = -1; cz <= 1; ++cz)
-#pragma unroll
-                    for (int cy = -1; cy <= 1; ++cy)
-#pragma unroll
-                        for (int cx = -1; cx <= 1; ++cx) {
-                            const int n2 = cx * cx + cy * cy + cz * cz;
-                            if (n2 == 0 || (Q == 19 && n2 == 3)) continue;
-                            const T w = T(6.0 * lattice_w<Q>(n2));
-                            const T* const pl = cz < 0 ? rm : cz == 0 ? rc : rp;
-                            const T f = pl[ro + cy * G::RBW + cx];
-                            if (cx) gx_ += T(cx) * w * f;
-                            if (cy) gy_ += T(cy) * w * f;
-                            if (cz) gz_ += T(cz) * w * f;
-                        }
-                const T g2 = gx_ * gx_ + gy_ * gy_ + gz_ * gz_;
-                const T ig = g2 > T(1e-10) ? rsqrt_t<T>(g2) : T(0);   // reading C8
-                const T g = g2 * ig;
-                const T nx = gx_ * ig, ny = gy_ * ig, nz = gz_ * ig;
-                T* const q = st + row * G::ROWP + C::OX - 1 + col;
-                const T sa = q[0], sxx = q[4 * C::BW], syy = q[5 * C::BW], szz = q[6 * C::BW];
-                const T rA = q[10 * C::BW];
-                const T rho = T(1) + icw * (sa + (sxx + syy + szz) * T(1.0 / 3.0));
-                const T Agc = cw * p.A * g;                               // c A |G|
-                q[0] = sa - Agc * T(0.5);                                 // a -= A|G| (1/3 + 1.5/9)
-                q[4 * C::BW] = sxx + T(0.5) * Agc * nx * nx;              // 4.5 (A/9)|G| n n
-                q[5 * C::BW] = syy + T(0.5) * Agc * ny * ny;
-                q[6 * C::BW] = szz + T(0.5) * Agc * nz * nz;
-                q[7 * C::BW] += Agc * nx * ny;                            // 9 (A/9)|G| n n
-                q[8 * C::BW] += Agc * nx * nz;
-                q[9 * C::BW] += Agc * ny * nz;
-                const T kap = cw * p.beta * rA * (T(1) - rA) * rho;       // c beta rhoA rhoB / rho
-                q[11 * C::BW] = kap * nx;
-                q[12 * C::BW] = kap * ny;
-                q[13 * C::BW] = kap * nz;
-                q[14 * C::BW] = p.A * g * T(1.0 / 3.0);                   // rest population (A/3)|G|
-            }
-        }
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // these writes precede the stage's next TMA fill
-        asm volatile("bar.sync 1, %0;" ::"n"(C::NT) : "memory");          // consumers only
+        mbar_wait(gdone(s), par);
         // ---- phase C: pull + projection over the fifteen fields ----
         int rs[C::NPT][3];
 #pragma unroll
@@ -344,9 +437,9 @@ struct Tma2gPlan final : Tma2gPlanBase {
         Tma2gParams<T> p;
         p.L = L; p.dst = (T*)dst; p.omega = T(omega); p.A = T(A); p.beta = T(beta); p.lz = lz;
         if (epi == EPI_SFORM)
-            kernel<EPI_SFORM>()<<<grid, C::NT + TMA_PRODUCER_THREADS, G::SMEM, stream>>>(row_map[from], ra2_map[from], ra8_map[from], p);
+            kernel<EPI_SFORM>()<<<grid, tma2g_threads(C::NT), G::SMEM, stream>>>(row_map[from], ra2_map[from], ra8_map[from], p);
         else
-            kernel<EPI_MOMENTS>()<<<grid, C::NT + TMA_PRODUCER_THREADS, G::SMEM, stream>>>(row_map[from], ra2_map[from], ra8_map[from], p);
+            kernel<EPI_MOMENTS>()<<<grid, tma2g_threads(C::NT), G::SMEM, stream>>>(row_map[from], ra2_map[from], ra8_map[from], p);
         return (int)cudaGetLastError();
     }
 
