@@ -319,7 +319,7 @@ struct Tma2gCtx final : lbwp_ctx {
     int export_dense(void* ext) override {
         if (steps == 0) {
             const dim3 b(32, 8, 1), g((X.nx + 31) / 32, (X.ny + 7) / 8, X.nz);
-            lbwp::k_tma2g_export_raw<T><<<g, b, 0, stream>>>(X, (const T*)buf[cur ^ 1], (T*)ext);
+            lbwp::k_tma2g_export_raw<T><<<g, b, 0, stream>>>(planp->Lb[cur ^ 1], (const T*)buf[cur ^ 1], (T*)ext);
             CU(cudaGetLastError());
             return LBWP_OK;
         }

@@ -17,9 +17,9 @@
 // lbwp_moments() gets the plain moments of time t by running the same stencil on the previous
 // ping-pong buffer (the S-form of time t-1) with an epilogue that writes rho, u, P instead.
 //
-// Layout ("XLayout"): field-major [10][nz][ny][px], x fastest; ghost columns in x only (x = -1 on the
-// left, x = nx and nx+1 on the right, written by the owners of their images); y and z wrap on the load
-// side (TMA coordinates).
+// Layout ("XLayout"): field-major [M][nz][ny][px], x fastest; ghost columns in x only (up to x = -2 on the
+// left and x = nx+2 on the right, written by the owners of their images; which of them a kernel maintains
+// and reads is its own business); y and z wrap on the load side (TMA coordinates).
 // Interior x = 0 sits 16 bytes into a row, rows are a multiple of 32 bytes.
 //
 // Mapping: a CTA owns a TX x TY tile of columns and marches over a chunk of z planes.  Each
@@ -49,7 +49,7 @@ inline XLayout make_xlayout(int nx, int ny, int nz, int elem_bytes) {
     L.nx = nx; L.ny = ny; L.nz = nz;
     L.ox = 16 / elem_bytes;
     const int q = 32 / elem_bytes;
-    L.px = ((L.ox + nx + 2 + q - 1) / q) * q;   // one ghost column left, two right
+    L.px = ((L.ox + nx + 3 + q - 1) / q) * q;   // ghost columns: x = -2, -1 on the left (ox >= 2), x = nx .. nx+2 on the right
     L.plane = (long long)L.px * ny;
     L.field = L.plane * nz;
     return L;

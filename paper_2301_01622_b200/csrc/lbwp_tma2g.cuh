@@ -37,8 +37,11 @@ struct Tma2gCfg {
     static constexpr uint32_t ROW_TX_BYTES = (uint32_t)(MT * BW * sizeof(T));
     // rA ring: box start 32 bytes left of the tile (halo 2 in x), rows of RBW elements with 2 rows = 128-byte multiple
     static constexpr int ROX = 32 / (int)sizeof(T);
+    // ring column of stage column 0: both boxes start at 16-byte aligned columns of the padded row, the ring's box
+    // RCO columns further left (x-paired mode: the stage box starts at x0 + 4, see TmaCfg, the ring box at x0)
+    static constexpr int RCO = C::PX ? 4 : ROX - OX;
     static constexpr int RBW = (TX + 2 * ROX + 64 / (int)sizeof(T) - 1) / (64 / (int)sizeof(T)) * (64 / (int)sizeof(T));
-    static constexpr int RROWS = TY + 4, RNS = 5;
+    static constexpr int RROWS = TY + 4, RNS = NS + 2;
     static constexpr int RPLANE = RROWS * RBW;
     static constexpr uint32_t RPLANE_TX_BYTES = (uint32_t)(RPLANE * sizeof(T));
     static constexpr size_t SMEM = (size_t)(NS * STAGE + RNS * RPLANE) * sizeof(T) + 3 * NS * 8 + 128;
@@ -53,6 +56,7 @@ struct Tma2gParams {
     T* __restrict__ dst;   // EPI_SFORM: 11 state fields (XLayout); EPI_MOMENTS: dense external [11][nz][ny][nx]
     T omega, A, beta;
     int lz;
+    int sh;                // x-paired mode: 1 if the CTA owns x0+1 .. x0+TX (reading buffer 0), else 0 (TmaCfg)
 };
 
 // finished sums (drho, j, dP_aa, P_ab, rhoA) of one node -> the eleven state fields (BGK in moment space, Eq. 8), with
@@ -69,8 +73,8 @@ __device__ __forceinline__ void store_state2g(const XLayout& L, T* __restrict__ 
     T* __restrict__ d = dst + xidx(L, x, y, z);
 #pragma unroll
     for (int f = 0; f < 11; ++f) d[f * F] = out[f];
-    if (x < 2 || x >= L.nx - 2) {
-        T* __restrict__ g = x < 2 ? d + L.nx : d - L.nx;
+    if (x < 3 || x >= L.nx - 2) {   // images at x = nx, nx+1, nx+2 and x = -2, -1
+        T* __restrict__ g = x < 3 ? d + L.nx : d - L.nx;
 #pragma unroll
         for (int f = 0; f < 11; ++f) g[f * F] = out[f];
     }
@@ -78,16 +82,52 @@ __device__ __forceinline__ void store_state2g(const XLayout& L, T* __restrict__ 
 
 // ---- phase G of one unit = GN x-adjacent source nodes (fp32: a pair, all arithmetic packed; fp64: one node) ----
 // st: main stage, ring planes rm / rc / rp = rA at z-1, z, z+1; row slot 0 .. TY+1, col 0 <-> x0 - 1 (col even for GN = 2)
+// x-paired fp32 nodes (x, x+1): packed collision, one 8-byte store per field (the destination buffer's parity makes
+// the pair aligned, see TmaCfg), then the periodic images element by element: x = nx-2, nx-1 also at x - nx; x = 0, 1, 2
+// also at x + nx (reading buffer 0 the stencil reaches x = nx+2, reading buffer 1 x = -2); the pair (nx-1, nx) holds
+// node 0 in its second element, whose image at x - nx is node 0's home column.
+template <int Q>
+__device__ __forceinline__ void store_state2g_pair(const XLayout& L, float* __restrict__ dst, const f32x2 (&a)[11], float omega,
+                                                   int x, int y, int z) {
+    f32x2 out[11];
+    collide_sform_v<float, f32x2, 2, Q>(reinterpret_cast<const f32x2(&)[10]>(a), omega, reinterpret_cast<f32x2(&)[10]>(out));
+    out[10].x = a[10].x * __frcp_rn(1.0f + a[0].x);
+    out[10].y = a[10].y * __frcp_rn(1.0f + a[0].y);
+    const long long F = L.field;
+    float* __restrict__ d = dst + xidx(L, x, y, z);
+#pragma unroll
+    for (int f = 0; f < 11; ++f) *reinterpret_cast<float2*>(d + f * F) = make_float2(out[f].x, out[f].y);
+    if (x < 3 || x + 1 >= L.nx - 2) {
+#pragma unroll
+        for (int n = 0; n < 2; ++n) {
+            const int xe = x + n;
+            if (xe < 3 || xe >= L.nx - 2) {
+                float* __restrict__ e = d + n + (xe < 3 ? L.nx : -L.nx);
+#pragma unroll
+                for (int f = 0; f < 11; ++f) e[f * F] = n ? out[f].y : out[f].x;
+            }
+        }
+    }
+}
+template <int Q, typename V>
+__device__ __forceinline__ void store_state2g_pair(const XLayout&, double*, const V (&)[11], double, int, int, int) {}
+
 template <typename T, typename C, typename G, int GN>
 __device__ __forceinline__ void colour_unit(T* __restrict__ st, const T* __restrict__ rm, const T* __restrict__ rc,
                                             const T* __restrict__ rp, int row, int col, T A, T beta) {
     using GV = Vec<T, GN>;
     constexpr int Q = C::Q;
-    const int ro = (row + 1) * G::RBW + G::ROX - 1 + col;     // ring: row 0 <-> y0 - 2, column ROX <-> x0
+    const int sc = C::OX - 1 + col;                              // stage column of the unit's first node
+    const int ro = (row + 1) * G::RBW + G::RCO + sc;             // ring: row 0 <-> y0 - 2
     // the three x taps of one ring row for the unit's nodes: m = f(x-1), c = f(x), p = f(x+1)
     auto taps = [&](const T* __restrict__ pl, int dy, GV& m, GV& c, GV& p) {
         const T* __restrict__ q = pl + ro + dy * G::RBW;
-        if constexpr (GN == 2) {   // ro is odd: (x-1, x) and (x+1, x+2) are the two aligned 8-byte pairs
+        if constexpr (GN == 2 && C::PX != 0) {   // ro is even: the pair itself is the aligned 8-byte load
+            const float l = q[-1];
+            const float2 b = *reinterpret_cast<const float2*>(q);
+            const float h = q[2];
+            m.x = l; m.y = b.x; c.x = b.x; c.y = b.y; p.x = b.y; p.y = h;
+        } else if constexpr (GN == 2) {          // ro is odd: (x-1, x) and (x+1, x+2) are the two aligned 8-byte pairs
             const float2 a = *reinterpret_cast<const float2*>(q - 1), b = *reinterpret_cast<const float2*>(q + 1);
             m.x = a.x; m.y = a.y; c.x = a.y; c.y = b.x; p.x = b.x; p.y = b.y;
         } else {
@@ -141,26 +181,30 @@ __device__ __forceinline__ void colour_unit(T* __restrict__ st, const T* __restr
 #pragma unroll
     for (int n = 0; n < GN; ++n) ig.set(n, g2.get(n) > T(1e-10) ? rsqrt_t<T>(g2.get(n)) : T(0));   // reading C8
     const GV g = g2 * ig, nx = gx * ig, ny = gy * ig, nz = gz * ig;
-    T* __restrict__ q = st + row * G::ROWP + C::OX - 1 + col;
+    T* __restrict__ q = st + row * G::ROWP + sc;
     // Away from the interface (n = 0 for every node of the warp's units, reading C8) both colour operators vanish
     // identically: the S-form stays as it is and K = R0 = 0.  Exact, warp-uniform, and the common case.
     bool flat = true;
 #pragma unroll
     for (int n = 0; n < GN; ++n) flat = flat && ig.get(n) == T(0);
-    if (__all_sync(__activemask(), flat)) {
-#pragma unroll
-        for (int f = 11; f < 15; ++f)
-#pragma unroll
-            for (int n = 0; n < GN; ++n) q[f * C::BW + n] = T(0);
-        return;
-    }
     auto ldv = [&](int f) { GV v;
+        if constexpr (GN == 2 && C::PX != 0) { const float2 w = *reinterpret_cast<const float2*>(q + f * C::BW); v.x = w.x; v.y = w.y; }
+        else {
 #pragma unroll
-        for (int n = 0; n < GN; ++n) v.set(n, q[f * C::BW + n]);
+            for (int n = 0; n < GN; ++n) v.set(n, q[f * C::BW + n]);
+        }
         return v; };
     auto stv = [&](int f, const GV& v) {
+        if constexpr (GN == 2 && C::PX != 0) *reinterpret_cast<float2*>(q + f * C::BW) = make_float2(v.get(0), v.get(1));
+        else {
 #pragma unroll
-        for (int n = 0; n < GN; ++n) q[f * C::BW + n] = v.get(n); };
+            for (int n = 0; n < GN; ++n) q[f * C::BW + n] = v.get(n);
+        } };
+    if (__all_sync(__activemask(), flat)) {
+#pragma unroll
+        for (int f = 11; f < 15; ++f) stv(f, GV::bc(T(0)));
+        return;
+    }
     const T cw = Q == 27 ? T(1.0 / 216.0) : T(1.0 / 36.0);
     const GV sa = ldv(0), sxx = ldv(4), syy = ldv(5), szz = ldv(6), rA = ldv(10);
     const GV rho = vfma(GV::bc(T(1) / cw), vfma(GV::bc(T(1.0 / 3.0)), sxx + syy + szz, sa), GV::bc(T(1)));
@@ -230,7 +274,8 @@ k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant_
         if (tid != C::NT + TMA2G_G_THREADS) return;
         auto wrapz = [&](int z) { return z < 0 ? z + L.nz : (z >= L.nz ? z - L.nz : z); };
         auto wrapy = [&](int y) { return y < 0 ? y + L.ny : (y >= L.ny ? y - L.ny : y); };
-        const int bx = t.x0 + L.ox - C::OX, rbx = t.x0 + L.ox - G::ROX;
+        const int bx = C::PX ? t.x0 + 16 / (int)sizeof(T) : t.x0 + L.ox - C::OX;   // stage box start column (16-byte aligned)
+        const int rbx = bx - G::RCO;
         // rA plane of relative index i (plane z0 - 1 + i) -> ring slot (i + 1) % RNS
         auto load_ra = [&](int i, uint32_t bar) {
             const int z = wrapz(wrapz(t.z0 - 1 + i));
@@ -285,12 +330,14 @@ k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant_
     // ---- consumer warps: phases C and E ----
     setmaxnreg_inc<tma2g_consumer_regs(C::NT)>();
     const int tc = tid % C::COLS_T, tr = tid / C::COLS_T;
-    constexpr int DY = C::ROWS_T;
+    // node n of the thread: column tx + n * DX, row tr + n * DY of the tile (x-paired: the pair 2 tc, 2 tc + 1)
+    constexpr int DX = C::PX ? 1 : 0, DY = C::PX ? 0 : C::ROWS_T;
+    const int tx = C::PX ? 2 * tc : tc;
     int r[C::NPT][3];   // element offsets (within a stage) of the three source rows of each owned node
 #pragma unroll
     for (int n = 0; n < C::NPT; ++n)
 #pragma unroll
-        for (int j = 0; j < 3; ++j) r[n][j] = (tr + n * DY + j) * G::ROWP + C::OX + tc;
+        for (int j = 0; j < 3; ++j) r[n][j] = (tr + n * DY + j) * G::ROWP + C::OX + tx + n * DX;
 
     V a0[C::NA], a1[C::NA], a2[C::NA];
 #pragma unroll
@@ -312,13 +359,19 @@ k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant_
         consumer_release(empty(s), tid);
         // ---- phase E: this input plane completes output plane z0 + i - 2 ----
         if (i >= 2) {
+            if constexpr (C::PX != 0 && EPI == EPI_SFORM) {
+                store_state2g_pair<Q>(L, p.dst, P, p.omega, t.x0 + p.sh + tx, t.y0 + tr, t.z0 + i - 2);
+            } else {
 #pragma unroll
-            for (int n = 0; n < C::NPT; ++n) {
-                T acc[C::NA];
+                for (int n = 0; n < C::NPT; ++n) {
+                    T acc[C::NA];
 #pragma unroll
-                for (int f = 0; f < C::NA; ++f) acc[f] = P[f].get(n);
-                if (EPI == EPI_SFORM) store_state2g<T, Q>(L, p.dst, acc, p.omega, t.x0 + tc, t.y0 + tr + n * DY, t.z0 + i - 2);
-                else store_dense2<T>(L, p.dst, acc, t.x0 + tc, t.y0 + tr + n * DY, t.z0 + i - 2);
+                    for (int f = 0; f < C::NA; ++f) acc[f] = P[f].get(n);
+                    int x = t.x0 + p.sh + tx + n * DX;
+                    if (x == L.nx) x = 0;   // x-paired mode: the last pair of a row ends on node 0
+                    if (EPI == EPI_SFORM) store_state2g<T, Q>(L, p.dst, acc, p.omega, x, t.y0 + tr + n * DY, t.z0 + i - 2);
+                    else store_dense2<T>(L, p.dst, acc, x, t.y0 + tr + n * DY, t.z0 + i - 2);
+                }
             }
         }
         if (++s == G::NS) { s = 0; par ^= 1u; }
@@ -337,7 +390,7 @@ k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant_
 
 // dense external moments [11][nz][ny][nx] (rhoA, rhoB, u, P) -> the eleven state fields, and a plain copy for t = 0
 template <typename T, int Q>
-__global__ void __launch_bounds__(256) k_tma2g_import(XLayout L, const T* __restrict__ ext, T* __restrict__ state,
+__global__ void __launch_bounds__(256) k_tma2g_import(XLayout L, XLayout Lraw, const T* __restrict__ ext, T* __restrict__ state,
                                                       T* __restrict__ raw, T omega) {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
@@ -345,7 +398,7 @@ __global__ void __launch_bounds__(256) k_tma2g_import(XLayout L, const T* __rest
     if (x >= L.nx || y >= L.ny) return;
     const long long n = (long long)L.nx * L.ny * L.nz;
     const long long e = ((long long)z * L.ny + y) * L.nx + x;
-    const long long F = L.field, c = xidx(L, x, y, z);
+    const long long F = L.field, c = xidx(Lraw, x, y, z);
     T m[11];
 #pragma unroll
     for (int f = 0; f < 11; ++f) { m[f] = ext[f * n + e]; raw[f * F + c] = m[f]; }
@@ -374,10 +427,11 @@ __global__ void __launch_bounds__(256) k_tma2g_export_raw(XLayout L, const T* __
 
 // ---- host side ---------------------------------------------------------------------------------------
 template <typename T, int Q> struct Tma2gGeom;
-template <int Q> struct Tma2gGeom<float, Q> { using C = TmaCfg<float, 2, 64, 8, 3, Q, 2>; };
-template <int Q> struct Tma2gGeom<double, Q> { using C = TmaCfg<double, 1, 32, 8, 3, Q, 2>; };
+template <int Q> struct Tma2gGeom<float, Q> { using C = TmaCfg<float, 2, 64, 8, 4, Q, 2, Q == 19 ? 1 : 0>; };
+template <int Q> struct Tma2gGeom<double, Q> { using C = TmaCfg<double, 1, 32, 8, 4, Q, 2>; };
 
 struct Tma2gPlanBase {
+    XLayout Lb[2];   // per buffer: the x-paired fp32 kernel keeps buffer 1 one column to the right (TmaCfg)
     virtual ~Tma2gPlanBase() {}
     virtual int setup(const XLayout& L_, void* const buf[2]) = 0;
     virtual int stencil(int epi, int from, void* dst, double omega, double A, double beta, cudaStream_t stream) const = 0;
@@ -413,6 +467,8 @@ struct Tma2gPlan final : Tma2gPlanBase {
 
     int setup(const XLayout& L_, void* const buf[2]) override {
         L = L_;
+        Lb[0] = Lb[1] = L;
+        if (C::PX) Lb[1].ox += 1;
         for (int k = 0; k < 2; ++k) {
             int rc = make_box_map<T>(&row_map[k], buf[k], L, 11, C::BW, G::MT, 1);
             if (!rc) rc = make_box_map<T>(&ra2_map[k], buf[k], L, 11, G::RBW, 1, 2);
@@ -435,7 +491,8 @@ struct Tma2gPlan final : Tma2gPlanBase {
     // one pass from buffer `from`: EPI_SFORM -> the eleven state fields of dst, EPI_MOMENTS -> dense moments in dst
     int stencil(int epi, int from, void* dst, double omega, double A, double beta, cudaStream_t stream) const override {
         Tma2gParams<T> p;
-        p.L = L; p.dst = (T*)dst; p.omega = T(omega); p.A = T(A); p.beta = T(beta); p.lz = lz;
+        p.L = Lb[from ^ 1]; p.dst = (T*)dst; p.omega = T(omega); p.A = T(A); p.beta = T(beta); p.lz = lz;   // EPI_SFORM writes the other buffer
+        p.sh = (C::PX && from == 0) ? 1 : 0;
         if (epi == EPI_SFORM)
             kernel<EPI_SFORM>()<<<grid, tma2g_threads(C::NT), G::SMEM, stream>>>(row_map[from], ra2_map[from], ra8_map[from], p);
         else
@@ -445,7 +502,7 @@ struct Tma2gPlan final : Tma2gPlanBase {
 
     int import_state(const void* ext, void* state, void* raw, double omega, cudaStream_t stream) const override {
         const dim3 b(32, 8, 1), g((L.nx + 31) / 32, (L.ny + 7) / 8, L.nz);
-        k_tma2g_import<T, Q><<<g, b, 0, stream>>>(L, (const T*)ext, (T*)state, (T*)raw, T(omega));
+        k_tma2g_import<T, Q><<<g, b, 0, stream>>>(Lb[0], Lb[1], (const T*)ext, (T*)state, (T*)raw, T(omega));
         return (int)cudaGetLastError();
     }
 };

@@ -27,7 +27,7 @@ struct TmaStepParams {
 template <typename T, int NPT_, int TX_, int TY_, int NS_, int Q_ = 27, int NC_ = 1, int PX_ = 0>
 struct TmaCfg {
     static constexpr int NPT = NPT_, TX = TX_, TY = TY_, NS = NS_, Q = Q_, NC = NC_, PX = PX_;
-    static_assert(PX_ == 0 || (NPT_ == 2 && sizeof(T) == 4 && NC_ == 1), "x-paired mode: fp32, two nodes, one component");
+    static_assert(PX_ == 0 || (NPT_ == 2 && sizeof(T) == 4), "x-paired mode: fp32, two nodes");
     static constexpr int M = NC_ == 1 ? 10 : 15;                    // fields per node in a stage
     static constexpr int NA = NC_ == 1 ? 10 : 11;                   // moment sums per node
     static_assert(Q_ == 27 || Q_ == 19, "lattice");
@@ -267,6 +267,19 @@ struct TmaStep {
         P[8] = P[8] - n10; P[9] = P[9] - n01;
     }
 
+    // the three x taps of field F in row slot j, as populations see them: k[2] = source x-1 (cx = +1), k[1] = source x
+    // (cx = 0), k[0] = source x+1 (cx = -1); either mode
+    template <int F>
+    __device__ static __forceinline__ void ld3any(const T* __restrict__ s, const int (&r)[C::NPT][3], int j, V (&k)[3]) {
+        if constexpr (C::PX != 0) ld3<F>(s, r[0][j], k[2], k[1], k[0]);
+        else { k[0] = ld<F, -1>(s, r, j); k[1] = ld<F, 0>(s, r, j); k[2] = ld<F, 1>(s, r, j); }
+    }
+    template <int F>
+    __device__ static __forceinline__ V ld1any(const T* __restrict__ s, const int (&r)[C::NPT][3], int j) {
+        if constexpr (C::PX != 0) return ldm<F>(s, r[0][j]);
+        else return ld<F, 0>(s, r, j);
+    }
+
     // consume one S-form input plane z: last contribution to output plane z-1 (P), middle one to
     // plane z (C), first one to plane z+1 (N, assigned).  Order: rho, jx, jy, jz, pxx, pyy, pzz, pxy, pxz, pyz
     __device__ static __forceinline__ void consume(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
@@ -303,7 +316,8 @@ struct TmaStep {
                                                       const V (&W)[3], const V (&O)[3], const V& four, V& ae, V& aw, V& ao) {
         constexpr int J = 1 - CY;
         const V cc = V::bc(C::Q == 27 ? T(1.0 / 216.0) : T(1.0 / 36.0));
-        const V ra[3] = {ld<10, -1>(s, r, J), ld<10, 0>(s, r, J), ld<10, 1>(s, r, J)};
+        V ra[3];
+        ld3any<10>(s, r, J, ra);
         V AE[3], AW[3], AO[3];
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
@@ -321,9 +335,9 @@ struct TmaStep {
                                                      V (&Cc)[C::NA], V (&N)[C::NA]) {
         const V four = V::bc(T(4));
         V El[3], Wl[3], Ol[3], Em[3], Wm[3], Om[3], Eh[3], Wh[3], Oh[3];
-        brackets<-1, true>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
-        brackets<1, true>(s, r, Eh, Wh, Oh);    // sources at y-1 (cy = +1)
-        brackets<0, true>(s, r, Em, Wm, Om);
+        brackets_any<-1, true>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
+        brackets_any<1, true>(s, r, Eh, Wh, Oh);    // sources at y-1 (cy = +1)
+        brackets_any<0, true>(s, r, Em, Wm, Om);
         {   // total fluid: as in consume()
             const Mom6<V> me = ypass<V>(xpass<V>(El[0], El[1], El[2], four), xpass<V>(Em[0], Em[1], Em[2], four),
                                         xpass<V>(Eh[0], Eh[1], Eh[2], four), four);
@@ -340,20 +354,24 @@ struct TmaStep {
         colour_row<0>(s, r, Em, Wm, Om, four, aem, awm, aom);
         const V mae = vfma(four, aem, aeh + ael), maw = vfma(four, awm, awh + awl), mao = vfma(four, aom, aoh + aol);
         // second part: sum_{c != 0} w_c K.c / |c|; weights x 216 / |c|: 16 (axis), 4/sqrt2 (face), 1/sqrt3 (corner)
-        const V kxa = ld<11, 1>(s, r, 1) - ld<11, -1>(s, r, 1);
-        const V kxb = (ld<11, 1>(s, r, 0) - ld<11, -1>(s, r, 0)) + (ld<11, 1>(s, r, 2) - ld<11, -1>(s, r, 2));
-        const V kya = ld<12, 0>(s, r, 0) - ld<12, 0>(s, r, 2);          // cy = +1 is row slot 0 (source y-1)
-        const V kyb = (ld<12, 1>(s, r, 0) - ld<12, 1>(s, r, 2)) + (ld<12, -1>(s, r, 0) - ld<12, -1>(s, r, 2));
-        const V z0 = ld<13, 0>(s, r, 1);
-        const V z1 = (ld<13, 1>(s, r, 1) + ld<13, -1>(s, r, 1)) + (ld<13, 0>(s, r, 0) + ld<13, 0>(s, r, 2));
-        const V z2 = (ld<13, 1>(s, r, 0) + ld<13, -1>(s, r, 0)) + (ld<13, 1>(s, r, 2) + ld<13, -1>(s, r, 2));
+        V kx0[3], kx1[3], kx2[3], ky0[3], ky2[3], kz0[3], kz1[3], kz2[3];   // K_a at row slot 0 (cy = +1), 1, 2
+        ld3any<11>(s, r, 0, kx0); ld3any<11>(s, r, 1, kx1); ld3any<11>(s, r, 2, kx2);
+        ld3any<12>(s, r, 0, ky0); ld3any<12>(s, r, 2, ky2);
+        ld3any<13>(s, r, 0, kz0); ld3any<13>(s, r, 1, kz1); ld3any<13>(s, r, 2, kz2);
+        const V kxa = kx1[2] - kx1[0];
+        const V kxb = (kx0[2] - kx0[0]) + (kx2[2] - kx2[0]);
+        const V kya = ky0[1] - ky2[1];
+        const V kyb = (ky0[2] - ky2[2]) + (ky0[0] - ky2[0]);
+        const V z0 = kz1[1];
+        const V z1 = (kz1[2] + kz1[0]) + (kz0[1] + kz2[1]);
+        const V z2 = (kz0[2] + kz0[0]) + (kz2[2] + kz2[0]);
         const V da = kxa + kya, db = kxb + kyb;
         const V f1 = V::bc(T(16)), f2 = V::bc(T(2.8284271247461903)), f3 = V::bc(T(0.57735026918962576));
         const V t0 = vfma(f1, da, f2 * db);                       // cz = 0
         const V tin = vfma(f2, da, f3 * db);                      // cz = +-1, in-plane part
         const V tz = vfma(f1, z0, vfma(f2, z1, f3 * z2));         // cz = +-1, c_z K_z part
         // rest population of the perturbation: to rho and (times rA) to rhoA of the node itself
-        const V r0 = ld<14, 0>(s, r, 1), rac = ld<10, 0>(s, r, 1);
+        const V r0 = ld1any<14>(s, r, 1), rac = ld1any<10>(s, r, 1);
         Cc[0] = Cc[0] + r0;
         Cc[10] = vfma(four, mae, Cc[10]) + vfma(rac, r0, t0);
         N[10] = (maw + mao) + (tin + tz);
@@ -366,7 +384,8 @@ struct TmaStep {
                                                            const V (&E)[3], const V (&W)[3], const V (&O)[3], bool sides,
                                                            V (&AE)[3], V (&AW)[3], V (&AO)[3]) {
         const V cc = V::bc(T(1.0 / 36.0));
-        const V ra[3] = {ld<10, -1>(s, r, j), ld<10, 0>(s, r, j), ld<10, 1>(s, r, j)};
+        V ra[3];
+        ld3any<10>(s, r, j, ra);
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
             const V rac = ra[k] * cc;
@@ -379,9 +398,9 @@ struct TmaStep {
                                                        V (&Cc)[C::NA], V (&N)[C::NA]) {
         const V two = V::bc(T(2)), eight = V::bc(T(8));
         V El[3], Wl[3], Ol[3], Em[3], Wm[3], Om[3], Eh[3], Wh[3], Oh[3];
-        brackets<-1, false>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
-        brackets<1, false>(s, r, Eh, Wh, Oh);    // sources at y-1 (cy = +1)
-        brackets<0, false>(s, r, Em, Wm, Om);
+        brackets_any<-1, false>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
+        brackets_any<1, false>(s, r, Eh, Wh, Oh);    // sources at y-1 (cy = +1)
+        brackets_any<0, false>(s, r, Em, Wm, Om);
         scatter19(El, Wl, Ol, Em, Wm, Om, Eh, Wh, Oh, P, Cc, N);   // total fluid: as in consume19()
         // colour A, first part: sum_c w_c rA (1 + B_c)
         V AEl[3], AWl[3], AOl[3], AEm[3], AWm[3], AOm[3], AEh[3], AWh[3], AOh[3];
@@ -394,18 +413,22 @@ struct TmaStep {
         const V maw = vfma(two, AWm[1], (AWm[2] + AWm[0]) + (AWh[1] + AWl[1]));
         const V mao = vfma(two, AOm[1], (AOm[2] + AOm[0]) + (AOh[1] + AOl[1]));
         // second part: sum_{c != 0} w_c K.c / |c|; weights x 36 / |c|: 2 (axis), 1/sqrt2 (face diagonal)
-        const V kxa = ld<11, 1>(s, r, 1) - ld<11, -1>(s, r, 1);
-        const V kxb = (ld<11, 1>(s, r, 0) - ld<11, -1>(s, r, 0)) + (ld<11, 1>(s, r, 2) - ld<11, -1>(s, r, 2));
-        const V kya = ld<12, 0>(s, r, 0) - ld<12, 0>(s, r, 2);
-        const V kyb = (ld<12, 1>(s, r, 0) - ld<12, 1>(s, r, 2)) + (ld<12, -1>(s, r, 0) - ld<12, -1>(s, r, 2));
-        const V z0 = ld<13, 0>(s, r, 1);
-        const V z1 = (ld<13, 1>(s, r, 1) + ld<13, -1>(s, r, 1)) + (ld<13, 0>(s, r, 0) + ld<13, 0>(s, r, 2));
+        V kx0[3], kx1[3], kx2[3], ky0[3], ky2[3], kz1[3];
+        ld3any<11>(s, r, 0, kx0); ld3any<11>(s, r, 1, kx1); ld3any<11>(s, r, 2, kx2);
+        ld3any<12>(s, r, 0, ky0); ld3any<12>(s, r, 2, ky2);
+        ld3any<13>(s, r, 1, kz1);
+        const V kxa = kx1[2] - kx1[0];
+        const V kxb = (kx0[2] - kx0[0]) + (kx2[2] - kx2[0]);
+        const V kya = ky0[1] - ky2[1];
+        const V kyb = (ky0[2] - ky2[2]) + (ky0[0] - ky2[0]);
+        const V z0 = kz1[1];
+        const V z1 = (kz1[2] + kz1[0]) + (ld1any<13>(s, r, 0) + ld1any<13>(s, r, 2));
         const V da = kxa + kya, db = kxb + kyb;
         const V f2 = V::bc(T(0.70710678118654752));
         const V t0 = vfma(two, da, f2 * db);     // cz = 0: axis and in-plane face diagonals
         const V tin = f2 * da;                   // cz = +-1: (+-1, 0, cz), (0, +-1, cz)
         const V tz = vfma(two, z0, f2 * z1);     // cz = +-1: c_z K_z of (0,0,cz) and the four above
-        const V r0 = ld<14, 0>(s, r, 1), rac = ld<10, 0>(s, r, 1);
+        const V r0 = ld1any<14>(s, r, 1), rac = ld1any<10>(s, r, 1);
         Cc[0] = Cc[0] + r0;
         Cc[10] = (Cc[10] + mae) + vfma(rac, r0, t0);
         N[10] = (maw + mao) + (tin + tz);
