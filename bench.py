@@ -10,8 +10,12 @@ config 5 instance D3Q27, single component, fp32, 512^3, seeded as config 1 (Tayl
 the two grid sizes the north star's target is stated on; both state buffers (2 x 5.4 GB) are far larger
 than L2, so no flush is needed between steps.  Prints ONE JSON line on stdout (rank 0).
 
-N > 1: the box is not decomposed in this round ("replicas only"): every rank advances its
-own box; value = all ranks' node updates / max-over-ranks device time; scaling = weak.
+The same line carries `sizes` (256^3 and 512^3, fp32 and fp64: MLUPS and the HBM fraction at each, as the north star
+asks), `footprint` (bytes per node and total GB with and without populations, from lbwp_state_bytes of both
+schemes) and `cpu_baseline` (the oracle on the host cores: all cores and single thread, 128^3).
+
+N > 1 (`--gpus N` under torchrun): every rank advances its own box ("replicas only" for the headline number,
+DESIGN.md); value = all ranks' node updates / max-over-ranks device time; scaling = weak.
 --impl reference: times the CPU oracle (oracle/, plain C fp64) on a bounded sample of the workload.
 """
 from __future__ import annotations
@@ -47,6 +51,8 @@ def parse_args():
     ap.add_argument("--kernel", default="auto", choices=["auto", "gather", "march", "tma", "tma_split"])
     ap.add_argument("--e2e-steps", type=int, default=2, help="host-buffer steps timed for the e2e key (0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sizes", action="store_true", help="skip the 256^3 / 512^3 fp32 / fp64 sub-record")
+    ap.add_argument("--size-steps", type=int, default=50, help="timed steps per entry of the sizes sub-record")
     return ap.parse_args()
 
 
@@ -74,7 +80,9 @@ def measured_peak():
 
 
 def ncu_traffic(kernel_name, n):
-    """dram read+write bytes per launch from the committed ncu capture (profiles/ncu_traffic.csv), or None."""
+    """dram read+write bytes per launch of this kernel at this size from the COMMITTED ncu --set full capture
+    (profiles/ncu_traffic.csv; its .md names the command and commit), or None.  Not measured in this run: ncu
+    cannot run inside a timed benchmark."""
     p = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     try:
         with open(p) as f:
@@ -131,25 +139,31 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def time_oracle(a, seconds_target=20.0):
-    """The oracle as it stands on the host cores: bounded sample of the workload's recipe."""
+def time_oracle(a, seconds_target=15.0, n=None, threads=None):
+    """The oracle as it stands on the host cores: a bounded sample of the workload's recipe (BASELINE.md section 3:
+    128^3; `threads` = None uses every core)."""
     import oracle
     from paper_2301_01622_b200 import workloads as wl
 
     oracle.build()
-    n = min(a.n, 96)
+    n = min(a.n, n or 128)
     cfg = wl.sweep_case(n, a.lattice, a.ncomp, "f64")
     m = cfg["moments"]
     fn = oracle.pop_run if a.scheme == "populations" else oracle.run
     kw = dict(lattice=a.lattice, ncomp=a.ncomp, tau=cfg["tau"], A=cfg["A"], beta=cfg["beta"])
-    t0 = time.perf_counter()
-    fn(m, nsteps=1, **kw)
-    t1 = time.perf_counter() - t0
-    steps = int(max(1, min(1000, seconds_target / max(t1, 1e-3))))
-    t0 = time.perf_counter()
-    fn(m, nsteps=steps, **kw)
-    dt = time.perf_counter() - t0
-    return {"value": n ** 3 * steps / dt / 1e6, "unit": METRIC, "cores": oracle.threads(), "kind": "oracle",
+    all_cores = oracle.set_threads(os.cpu_count() or 1)
+    used = oracle.set_threads(threads) if threads else all_cores
+    try:
+        t0 = time.perf_counter()
+        fn(m, nsteps=1, **kw)
+        t1 = time.perf_counter() - t0
+        steps = int(max(1, min(1000, seconds_target / max(t1, 1e-3))))
+        t0 = time.perf_counter()
+        fn(m, nsteps=steps, **kw)
+        dt = time.perf_counter() - t0
+    finally:
+        oracle.set_threads(all_cores)
+    return {"value": n ** 3 * steps / dt / 1e6, "unit": METRIC, "cores": used, "kind": "oracle",
             "sample": f"{n}^3 box of the same recipe, {steps} steps, fp64, {dt:.1f} s of host time"}, dt / steps, steps, n
 
 
@@ -185,10 +199,37 @@ def aggregate(per_rank_nodes_steps, max_ms):
     return sum(per_rank_nodes_steps) / (max_ms * 1e-3) / 1e6
 
 
+def time_steps(torch, sim, steps, warmup, barrier):
+    """W untimed steps, then exactly `steps` steps between two CUDA events on the launching stream."""
+    sim.step(max(3, warmup))
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    sim.step(steps)
+    ev1.record()
+    barrier()
+    return ev0.elapsed_time(ev1)
+
+
+def roofline_record(a_like, kname, nodes, ms, steps, lps, peak, peak_src):
+    """HBM roofline of one time step: algorithmic bytes (2 M sizeof per node) / measured step time.
+    A step is `lps` launches (1 for every moments kernel of the TMA path); launch_ms is the average launch."""
+    bpl = algorithmic_bytes_per_lu(a_like)
+    step_ms = ms / steps
+    achieved = bpl * nodes / (step_ms * 1e-3) / 1e9
+    return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "traffic": ncu_traffic(kname, a_like.n),
+            "traffic_source": "committed ncu --set full capture, profiles/ncu_traffic.csv (not measured in this run)",
+            "peak_source": peak_src, "algorithmic_bytes_per_node": bpl, "frac_of_8TBs_nominal": achieved / 8000.0,
+            "kernel": kname, "launches_per_step": lps, "step_ms": step_ms, "launch_ms": step_ms / lps}
+
+
 def main():
     a = parse_args()
     if a.impl == "reference":
         return run_reference(a)
+
+    import copy
 
     import torch
     import torch.distributed as dist
@@ -215,12 +256,16 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    cfg = wl.sweep_case(a.n, a.lattice, a.ncomp, a.dtype)
-    m0 = wl.as_dtype(cfg["moments"], a.dtype)
+    def make_sim(b):
+        cfg = wl.sweep_case(b.n, b.lattice, b.ncomp, b.dtype)
+        m0 = wl.as_dtype(cfg["moments"], b.dtype)
+        return lbwp.Lbwp(m0, lattice=b.lattice, dtype=b.dtype, ncomp=b.ncomp, tau=cfg["tau"], A=cfg["A"],
+                         beta=cfg["beta"], scheme=b.scheme, kernel=b.kernel, device=local), m0
+
+    peak, peak_src = measured_peak()
     nodes = a.n ** 3
-    sim = lbwp.Lbwp(m0, lattice=a.lattice, dtype=a.dtype, ncomp=a.ncomp, tau=cfg["tau"], A=cfg["A"],
-                    beta=cfg["beta"], scheme=a.scheme, kernel=a.kernel, device=local)
-    kname = sim.kernel_name
+    sim, m0 = make_sim(a)
+    kname, lps, state_bytes = sim.kernel_name, sim.launches_per_step, sim.state_bytes
     sim.step(max(3, a.warmup))
     barrier()
     sampler = ClockSampler(local)
@@ -229,12 +274,11 @@ def main():
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     ev0.record()
-    sim.step(a.steps)          # exactly K steps, K * launches_per_step kernel launches
+    sim.step(a.steps)          # exactly K steps, K * launches_per_step kernel launches, nothing else in the region
     ev1.record()
     barrier()
     clocks = sampler.stop()
-    ms = ev0.elapsed_time(ev1)
-    ms = max_over_ranks(ms, world, "cuda")
+    ms = max_over_ranks(ev0.elapsed_time(ev1), world, "cuda")
     value = aggregate([nodes * a.steps] * world, ms)
 
     # end-to-end through the C ABI with HOST buffers: every step uploads the state from pinned host
@@ -255,26 +299,55 @@ def main():
             sim.moments_host(out=h_out)     # synchronises
             h_in, h_out = h_out, h_in
         barrier()
-        dt = time.perf_counter() - t0
-        dt = max_over_ranks(dt, world, "cuda")
+        dt = max_over_ranks(time.perf_counter() - t0, world, "cuda")
         nbytes = h_in.numel() * h_in.element_size()
         e2e = {"value": nodes * a.e2e_steps * world / dt / 1e6, "unit": METRIC, "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes, "steps": a.e2e_steps,
                "what": "lbwp_set_moments(host) + lbwp_step(1) + lbwp_moments(host) per step, pinned host buffers"}
         del h_in, h_out
-    lps = sim.launches_per_step
-    state_bytes = sim.state_bytes
     sim.close()
+    del sim, m0
+
+    # the other sizes and precisions the north star names (rank 0, 1 GPU): same kernel path, fewer steps
+    sizes = None
+    if not a.no_sizes and world == 1 and a.scheme == "moments":
+        sizes = []
+        for n, dt in ((256, "f32"), (512, "f32"), (256, "f64"), (512, "f64")):
+            b = copy.copy(a)
+            b.n, b.dtype = n, dt
+            if (n, dt) == (a.n, a.dtype):
+                r = roofline_record(b, kname, nodes, ms, a.steps, lps, peak, peak_src)
+                steps = a.steps
+            else:
+                s2, _ = make_sim(b)
+                t = time_steps(torch, s2, a.size_steps, 5, barrier)
+                r = roofline_record(b, s2.kernel_name, n ** 3, t, a.size_steps, s2.launches_per_step, peak, peak_src)
+                steps = a.size_steps
+                s2.close()
+                del s2
+            sizes.append({"grid": n, "dtype": dt, "kernel": r["kernel"], "steps": steps,
+                          "mlups": r["algorithmic_bytes_per_node"] and r["achieved"] * 1e9 / r["algorithmic_bytes_per_node"] / 1e6,
+                          "achieved_gbs": r["achieved"], "frac": r["frac"], "frac_of_8TBs_nominal": r["frac_of_8TBs_nominal"]})
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
-    peak, peak_src = measured_peak()
-    bpl = algorithmic_bytes_per_lu(a)
-    launch_ms = ms / a.steps            # one dominant kernel launch per step
-    achieved = bpl * nodes / (launch_ms * 1e-3) / 1e9
-    traffic = ncu_traffic(kname, a.n)
+
+    # memory footprint with and without populations: what the library allocates for the state
+    def fp(scheme, ncomp):
+        p = lbwp.make_params(lattice=a.lattice, dtype=a.dtype, ncomp=ncomp, shape=(a.n,) * 3, tau=1.0, A=0.01, beta=0.7,
+                             scheme=scheme)
+        b = 2 * lbwp.state_bytes(p)          # two ping-pong buffers
+        return {"bytes_per_node": b / nodes, "total_gb": b / 1e9}
+    esz = 4 if a.dtype == "f32" else 8
+    footprint = {"grid": a.n, "dtype": a.dtype, "lattice": a.lattice,
+                 "moments_1c": fp("moments", 1), "moments_2c": fp("moments", 2),
+                 "populations_1c": fp("populations", 1), "populations_2c": fp("populations", 2),
+                 "ideal_bytes_per_node": {"moments_1c": 20 * esz, "moments_2c": 22 * esz,
+                                          "populations_1c": 2 * a.lattice * esz, "populations_2c": 4 * a.lattice * esz},
+                 "paper": "V100, 128^3, two-component D3Q19 fp32: 0.6782 GB without / 1.1411 GB with populations (PAPER.md:163)"}
+
     line = {
         "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": a.steps, "warmup": max(3, a.warmup),
         "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -285,13 +358,15 @@ def main():
         "clocks": clocks,
         "e2e": e2e,
         "gpu_launches": a.steps * lps,
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic, "peak_source": peak_src, "algorithmic_bytes_per_node": bpl,
-                     "frac_of_8TBs_nominal": achieved / 8000.0, "kernel": kname,
-                     "launch_ms": launch_ms},
+        "roofline": roofline_record(a, kname, nodes, ms, a.steps, lps, peak, peak_src),
+        "sizes": sizes,
+        "footprint": footprint,
+        "paper_context": "622 MLUPS without / 277 MLUPS with populations: V100 16 GB, 128^3, two-component D3Q19, fp32, with near-contact forces (PAPER.md:158-163); another machine and workload, not the target",
     }
     if not a.no_cpu_baseline and world == 1:
-        base, _, _, _ = time_oracle(a)
+        base, _, _, _ = time_oracle(a, seconds_target=12.0)
+        single, _, _, _ = time_oracle(a, seconds_target=8.0, threads=1)
+        base["single_thread"] = {"value": single["value"], "unit": METRIC, "cores": 1, "sample": single["sample"]}
         line["cpu_baseline"] = base
     elif not a.no_cpu_baseline:
         line["cpu_baseline"] = None

@@ -43,6 +43,7 @@ def _load():
         lib.lbwp_oracle_run.argtypes = run_args
         lib.lbwp_oracle_pop_run.argtypes = run_args
         lib.lbwp_oracle_threads.restype = ctypes.c_int
+        lib.lbwp_oracle_set_threads.argtypes, lib.lbwp_oracle_set_threads.restype = [ctypes.c_int], ctypes.c_int
         lib.lbwp_oracle_set_g2cut.argtypes = [ctypes.c_double]
         lib.lbwp_oracle_get_g2cut.restype = ctypes.c_double
         _lib = lib
@@ -56,6 +57,11 @@ def _dp(a: np.ndarray):
 def threads() -> int:
     """OpenMP threads the step loops will use (results do not depend on it)."""
     return int(_load().lbwp_oracle_threads())
+
+
+def set_threads(n: int) -> int:
+    """Use n OpenMP threads from now on (the single-thread / all-core timings of bench.py); returns what is set."""
+    return int(_load().lbwp_oracle_set_threads(int(n)))
 
 
 def set_g2cut(v: float) -> float:

@@ -341,6 +341,17 @@ int lbwp_oracle_threads(void) {
 #endif
 }
 
+/* number of threads the z loops use from now on (timing only: the results do not depend on it); returns what is set */
+int lbwp_oracle_set_threads(int n) {
+#ifdef _OPENMP
+    if (n >= 1) omp_set_num_threads(n);
+    return omp_get_max_threads();
+#else
+    (void)n;
+    return 1;
+#endif
+}
+
 /* ------------------------------------------------------------------------ */
 /* Mini-oracle of the COMPARISON kernel (standard LB "with populations",     */
 /* PAPER.md:29, 75, 163): two-lattice pull BGK on stored populations,        */

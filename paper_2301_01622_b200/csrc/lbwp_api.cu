@@ -30,6 +30,17 @@ int fail(int code, const char* fmt, ...) {
     return code;
 }
 
+// every entry point works on the context's device and leaves the caller's current device as it found it
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        if (prev != dev) ok = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 #define CU(call)                                                                               \
     do {                                                                                       \
         cudaError_t e_ = (call);                                                               \
@@ -47,6 +58,7 @@ bool params_ok(const lbwp_params* p) {
     if (p->kernel < LBWP_KERNEL_AUTO || p->kernel > LBWP_KERNEL_TMA_SPLIT) return false;
     if (p->nx < 1 || p->ny < 1 || p->nz < 1) return false;
     if ((long long)p->nx * p->ny * p->nz > (1ll << 31)) return false;
+    if (p->nz > 65535 || (p->ny + 7) / 8 > 65535) return false;   // the pointwise kernels put z (and y / 8) in gridDim.z (.y)
     if (!(p->tau > 0.5)) return false;  // also rejects NaN
     if ((p->buf[0] == nullptr) != (p->buf[1] == nullptr)) return false;
     return true;
@@ -333,7 +345,6 @@ size_t dense_bytes(const lbwp_ctx* c) { return (size_t)c->M * c->L.nx * c->L.ny 
 
 int load_moments(lbwp_ctx* c, const void* moments, int on_device) {
     if (!moments) return fail(LBWP_EINVAL, "moments is NULL");
-    CU(cudaSetDevice(c->P.device));
     const void* dev = moments;
     if (!on_device) {
         if (!c->staging) CU(cudaMalloc(&c->staging, dense_bytes(c)));
@@ -370,8 +381,8 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
     if (!moments) return fail(LBWP_EINVAL, "moments is NULL");
     const int variant = choose_variant(p);
     if (variant == 0)
-        return fail(LBWP_EUNSUPPORTED, "kernel %d is not built for this combination (MARCH: D3Q27 single-component; TMA: single-component "
-                    "moments; TMA also needs nx %% 64 (fp32) or 32 (fp64) == 0 and ny %% 8 == 0)", p->kernel);
+        return fail(LBWP_EUNSUPPORTED, "kernel %d is not built for this combination (MARCH: D3Q27 single-component moments; TMA: moments "
+                    "scheme with nx %% 64 (fp32) or 32 (fp64) == 0 and ny %% 8 == 0; TMA_SPLIT: two-component only)", p->kernel);
     int ndev = 0;
     CU(cudaGetDeviceCount(&ndev));
     if (p->device < 0 || p->device >= ndev) return fail(LBWP_EINVAL, "device %d out of range (%d devices)", p->device, ndev);
@@ -379,7 +390,8 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
     CU(cudaGetDeviceProperties(&prop, p->device));
     if (prop.major != 10)
         return fail(LBWP_EUNSUPPORTED, "device %d is sm_%d%d; this library is built for sm_100a only", p->device, prop.major, prop.minor);
-    CU(cudaSetDevice(p->device));
+    DeviceGuard guard(p->device);
+    if (!guard.ok) return fail(LBWP_ECUDA, "cudaSetDevice(%d) failed", p->device);
 
     lbwp_ctx* c = nullptr;
     if (variant == LBWP_KERNEL_TMA) {
@@ -435,6 +447,10 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
         if (e != cudaSuccess) return bail(fail(LBWP_ECUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e)));
     }
     c->variant = variant;
+    if (variant == LBWP_KERNEL_MARCH) {
+        const int e = p->dtype == LBWP_F32 ? lbwp::prepare_march27<float>() : lbwp::prepare_march27<double>();
+        if (e) return bail(fail(LBWP_ECUDA, "march kernel attribute: %s", cudaGetErrorString((cudaError_t)e)));
+    }
     if (variant == LBWP_KERNEL_TMA) {
         if (tma2_fused(p)) {
             rc = p->dtype == LBWP_F32 ? static_cast<Tma2gCtx<float>*>(c)->prepare() : static_cast<Tma2gCtx<double>*>(c)->prepare();
@@ -460,7 +476,8 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
 int lbwp_step(lbwp_ctx* c, int64_t n) {
     if (!c || n < 0) return fail(LBWP_EINVAL, "lbwp_step: ctx NULL or n < 0");
     if (n == 0) return LBWP_OK;
-    CU(cudaSetDevice(c->P.device));
+    DeviceGuard guard(c->P.device);
+    if (!guard.ok) return fail(LBWP_ECUDA, "cudaSetDevice(%d) failed", c->P.device);
     for (int64_t t = 0; t < n; ++t) {
         int rc = c->step_once();
         if (rc) return rc;
@@ -470,7 +487,8 @@ int lbwp_step(lbwp_ctx* c, int64_t n) {
 
 int lbwp_moments(lbwp_ctx* c, void* dst, int dst_on_device) {
     if (!c || !dst) return fail(LBWP_EINVAL, "lbwp_moments: NULL argument");
-    CU(cudaSetDevice(c->P.device));
+    DeviceGuard guard(c->P.device);
+    if (!guard.ok) return fail(LBWP_ECUDA, "cudaSetDevice(%d) failed", c->P.device);
     void* dev = dst;
     if (!dst_on_device) {
         if (!c->staging) CU(cudaMalloc(&c->staging, dense_bytes(c)));
@@ -485,6 +503,8 @@ int lbwp_moments(lbwp_ctx* c, void* dst, int dst_on_device) {
 
 int lbwp_set_moments(lbwp_ctx* c, const void* moments, int on_device) {
     if (!c) return fail(LBWP_EINVAL, "ctx is NULL");
+    DeviceGuard guard(c->P.device);
+    if (!guard.ok) return fail(LBWP_ECUDA, "cudaSetDevice(%d) failed", c->P.device);
     return load_moments(c, moments, on_device);
 }
 
@@ -494,13 +514,14 @@ const char* lbwp_kernel_name(const lbwp_ctx* c) { return c ? c->name : ""; }
 
 int lbwp_sync(lbwp_ctx* c) {
     if (!c) return fail(LBWP_EINVAL, "ctx is NULL");
+    DeviceGuard guard(c->P.device);
     CU(cudaStreamSynchronize(c->stream));
     return LBWP_OK;
 }
 
 int lbwp_destroy(lbwp_ctx* c) {
     if (!c) return LBWP_OK;
-    cudaSetDevice(c->P.device);
+    DeviceGuard guard(c->P.device);
     cudaStreamSynchronize(c->stream);
     if (c->owns)
         for (int k = 0; k < 2; ++k)

@@ -261,17 +261,20 @@ __global__ void __launch_bounds__(TX* TY, MINB) k_step_march27(const StepParams<
     }
 }
 
+// The fp64 instance needs more dynamic shared memory than the 48 KB default.  The attribute is per DEVICE, so it is
+// set by lbwp_init for the context's device (after cudaSetDevice), not once per process.
+template <typename T>
+int prepare_march27() {
+    constexpr int TX = 32, TY = 8, MINB = sizeof(T) == 4 ? 2 : 1;
+    return (int)cudaFuncSetAttribute(k_step_march27<T, TX, TY, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)March<T, TX, TY>::smem_bytes);
+}
+
 template <typename T>
 int launch_march27(const StepParams<T>& s, cudaStream_t stream) {
     constexpr int TX = 32, TY = 8, MINB = sizeof(T) == 4 ? 2 : 1;
     using K = March<T, TX, TY>;
     auto kern = k_step_march27<T, TX, TY, MINB>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::smem_bytes);
-        if (e != cudaSuccess) return (int)e;
-        attr_set = true;
-    }
     const int gx = (s.L.nx + TX - 1) / TX, gy = (s.L.ny + TY - 1) / TY;
     // z chunks: enough blocks to fill 148 SMs several times over, chunks >= 16 planes when possible
     int lz = s.L.nz;
@@ -279,7 +282,7 @@ int launch_march27(const StepParams<T>& s, cudaStream_t stream) {
     while ((long long)gx * gy * ((s.L.nz + lz - 1) / lz) < want && lz > 16) lz = (lz + 1) / 2;
     const dim3 grid(gx, gy, (s.L.nz + lz - 1) / lz), block(TX, TY, 1);
     kern<<<grid, block, K::smem_bytes, stream>>>(s, lz);
-    return 0;
+    return (int)cudaGetLastError();
 }
 
 }  // namespace lbwp

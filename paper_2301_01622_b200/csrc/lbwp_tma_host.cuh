@@ -2,7 +2,6 @@
 // pointwise import (moments -> S-form) and t = 0 export kernels of the XLayout state.
 #pragma once
 #include <cstdio>
-#include <cstdlib>
 #include <new>
 
 #include "lbwp_tma_kernel.cuh"
@@ -76,8 +75,7 @@ inline int make_state_map(CUtensorMap* out, const void* buf, const XLayout& L, i
                                    (cuuint64_t)L.plane * sizeof(T)};
     const cuuint32_t box[4] = {(cuuint32_t)bw, (cuuint32_t)nfields, (cuuint32_t)rows, 1};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
-    CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_128B;
-    if (const char* e = getenv("LBWP_TMA_L2PROMO")) promo = (CUtensorMapL2promotion)atoi(e);   // tuning override
+    const CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_128B;   // none / 64 / 256 B measured within 1 %
     const CUresult r = enc(out, sizeof(T) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4,
                            const_cast<void*>(buf), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                            CU_TENSOR_MAP_SWIZZLE_NONE, promo,
@@ -120,10 +118,6 @@ inline void tma_choose_chunks(int nz, long long cols, int ctas, int* lz, int* gz
         const double cost = (double)rounds * (l + 2) * (rounds == 1 ? 0.9 : 1.0);
         if (cost < best - 1e-9) { best = cost; *lz = l; *gz = g; }
     }
-    if (const char* e = getenv("LBWP_TMA_LZ")) {   // tuning override: planes per z chunk
-        const int l = atoi(e);
-        if (l >= 1) { *lz = l < nz ? l : nz; *gz = (nz + *lz - 1) / *lz; }
-    }
 }
 
 template <typename T, typename C, int MINB>
@@ -160,8 +154,6 @@ struct TmaPlanT final : TmaPlanBase {
         // one item per CTA: the hardware scheduler hands out items in order and keeps the frontier of
         // running items compact (a persistent grid with static striding measured 30 % slower at 512^3)
         grid = (int)items;
-        if (const char* e = getenv("LBWP_TMA_PERSIST"))
-            if (atoi(e) == 1) grid = (int)(items < resident ? items : resident);
         return 0;
     }
 
@@ -178,19 +170,8 @@ struct TmaPlanT final : TmaPlanBase {
 };
 
 // geometry lists: (nodes per thread, tile x, tile y, stages, min CTAs per SM, x-paired)
-#ifdef LBWP_F32_NPT   // tuning builds: a single fp32 geometry given on the command line
-#ifndef LBWP_F32_PX
-#define LBWP_F32_PX 0
-#endif
-#define LBWP_F32_LIST(X) X(LBWP_F32_NPT, LBWP_F32_TX, LBWP_F32_TY, LBWP_F32_NS, LBWP_F32_MINB, LBWP_F32_PX)
-#else
 #define LBWP_F32_LIST(X) X(2, 128, 8, 3, 1, 1) X(2, 64, 8, 3, 1, 1)
-#endif
-#ifdef LBWP_F64_NPT
-#define LBWP_F64_LIST(X) X(LBWP_F64_NPT, LBWP_F64_TX, LBWP_F64_TY, LBWP_F64_NS, LBWP_F64_MINB, 0)
-#else
 #define LBWP_F64_LIST(X) X(1, 64, 8, 3, 1, 0) X(1, 32, 8, 3, 1, 0)
-#endif
 
 // first geometry of the dtype's list whose tile divides the box; nullptr if none does
 template <typename T>

@@ -165,13 +165,8 @@ __host__ __device__ constexpr int tma_consumer_regs(int consumers, int minb) {
     const int r = (launch + (launch - TMA_PRODUCER_REGS) * TMA_PRODUCER_THREADS / consumers) / 8 * 8;
     return r > 248 ? 248 : r;
 }
-#ifdef LBWP_NO_SETMAXNREG
-template <int N> __device__ __forceinline__ void setmaxnreg_inc() {}
-template <int N> __device__ __forceinline__ void setmaxnreg_dec() {}
-#else
 template <int N> __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
-#endif
 
 template <typename T, typename C, int EPI, int MINB>
 __global__ void __maxnreg__(tma_max_regs(C::NT + TMA_PRODUCER_THREADS, MINB))

@@ -14,7 +14,7 @@ import os
 import numpy as np
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("LBWP_LIB") or os.path.join(_PKG, "liblbwp.so")   # LBWP_LIB: another build of the same ABI
+LIB_PATH = os.path.join(_PKG, "liblbwp.so")
 
 LBWP_F32, LBWP_F64 = 0, 1
 LBWP_MOMENTS, LBWP_POPULATIONS = 0, 1
@@ -152,13 +152,27 @@ class Lbwp:
         torch = self._torch
         if out is None:
             out = torch.empty((self.M, *self.shape), dtype=self.t_dtype, device=self.device)
+        self._check_out(out)
         _check(load().lbwp_moments(self._ctx, ctypes.c_void_p(out.data_ptr()), int(out.is_cuda)))
         return out
+
+    def _check_out(self, out):
+        """The library writes M*nz*ny*nx elements of the run's dtype: refuse anything else (no silent overrun)."""
+        shape = tuple(out.shape)
+        if isinstance(out, np.ndarray):
+            ok = out.dtype == self.np_dtype and out.flags["C_CONTIGUOUS"] and out.flags["WRITEABLE"]
+        else:
+            ok = out.dtype == self.t_dtype and out.is_contiguous()
+            if out.is_cuda and out.device != self.device:
+                ok = False
+        if not ok or shape != (self.M, *self.shape):
+            raise ValueError(f"out must be a contiguous [{self.M}, nz, ny, nx] = {(self.M, *self.shape)} array of {self.dtype}")
 
     def moments_host(self, out=None) -> np.ndarray:
         """lbwp_moments into a host numpy array (or a pinned torch CPU tensor passed as ``out``)."""
         if out is None:
             out = np.empty((self.M, *self.shape), dtype=self.np_dtype)
+        self._check_out(out)
         if isinstance(out, np.ndarray):
             _check(load().lbwp_moments(self._ctx, out.ctypes.data_as(ctypes.c_void_p), 0))
         else:
