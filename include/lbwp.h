@@ -93,15 +93,40 @@ int lbwp_num_moments(const lbwp_params *params);
  * before returning.  *out is set only on success. */
 int lbwp_init(const lbwp_params *params, const void *moments, int moments_on_device, lbwp_ctx **out);
 
-/* Enqueue n >= 0 time steps on the context's stream; asynchronous (no sync).
+/* Enqueue n >= 0 time steps on the context's stream; asynchronous (no sync).  One step = for every node x and
+ * direction c_i: Eq. 8 at x - c_i, pulled to x (Eq. 9), summed into the new moments
+ * (Eq. 1-3); ncomp == 2: with the colour-gradient perturbation and recolouring (C6).
  * n == 0 is a no-op.  Launch errors are reported; execution errors surface at the
  * next synchronising call. */
 int lbwp_step(lbwp_ctx *ctx, int64_t n);
 
-/* Write the current moments, external layout, M*nz*ny*nx elements of params.dtype,
+/* Write the current moments H = [rho, u_a, P_ab], i.e. the POST-STREAM, PRE-COLLISION moments of
+ * Eq. 1-3 at the current time (reading C5: Eq. 8-9 collide at the neighbour, then stream), external layout,
+ * M*nz*ny*nx elements of params.dtype,
  * to `dst` (HOST pointer if dst_on_device == 0, else DEVICE pointer).  Synchronises
  * the stream.  Does not change the state. */
 int lbwp_moments(lbwp_ctx *ctx, void *dst, int dst_on_device);
+
+/* The paper's run-time diagnostics of the CURRENT state (Fig. 2, 3, 5, 7), one fused reduction
+ * in fp64 over all nodes.  "Density" is the density of the first component (the droplet fluid, whose field ranges
+ * from 0 to 1): rhoA for ncomp == 2, rho for ncomp == 1.
+ *   mass[2]      sum over nodes of rhoA and of rhoB (0 for ncomp == 1)              (Eq. 1 summed over the box)
+ *   momentum[3]  sum over nodes of rho u, rho = rhoA + rhoB                          (Eq. 2 summed over the box)
+ *   rho_mean_above, count_above   <density>_{density > threshold} and the number of such nodes (the paper's
+ *                <rho>_{rho > 0.5}; mean is 0 if no node qualifies)
+ *   rho_max      maximum of the density (the paper's rho_N,MAX)
+ * probe_xyz: nprobes triples (x, y, z) of node coordinates (HOST pointer, may be NULL if nprobes == 0);
+ * probe_rho: the density at those nodes (HOST pointer).  Synchronises the stream; does not change the state.
+ * LBWP_EINVAL for a NULL argument, nprobes < 0 or a probe outside the box. */
+typedef struct lbwp_diag {
+    double mass[2];
+    double momentum[3];
+    double rho_mean_above;
+    double rho_max;
+    int64_t count_above;
+} lbwp_diag;
+int lbwp_diagnostics(lbwp_ctx *ctx, double threshold, int nprobes, const int32_t *probe_xyz, lbwp_diag *out,
+                     double *probe_rho);
 
 /* Replace the state by new moments (same conventions as lbwp_init); step counter -> 0. */
 int lbwp_set_moments(lbwp_ctx *ctx, const void *moments, int moments_on_device);

@@ -43,6 +43,7 @@ def _load():
         lib.lbwp_oracle_run.argtypes = run_args
         lib.lbwp_oracle_pop_run.argtypes = run_args
         lib.lbwp_oracle_threads.restype = ctypes.c_int
+        lib.lbwp_oracle_diagnostics.argtypes = [ctypes.c_int] * 4 + [dp, ctypes.c_double, ctypes.c_int, ip, dp, dp]
         lib.lbwp_oracle_set_threads.argtypes, lib.lbwp_oracle_set_threads.restype = [ctypes.c_int], ctypes.c_int
         lib.lbwp_oracle_set_g2cut.argtypes = [ctypes.c_double]
         lib.lbwp_oracle_get_g2cut.restype = ctypes.c_double
@@ -123,3 +124,18 @@ def pop_run(moments, *, lattice: int, ncomp: int = 1, tau: float, nsteps: int, A
             beta: float = 0.0) -> np.ndarray:
     """Same interface, population-storing BGK (the comparison kernel's mini-oracle)."""
     return _run(_load().lbwp_oracle_pop_run, moments, lattice, ncomp, tau, nsteps, A, beta)
+
+
+def diagnostics(moments, *, ncomp: int = 1, threshold: float = 0.5, probes=()) -> dict:
+    """The paper's diagnostics of a state [M,nz,ny,nx]; probes = [(x, y, z), ...]."""
+    m = np.ascontiguousarray(moments, dtype=np.float64)
+    _, nz, ny, nx = m.shape
+    n = len(probes)
+    xyz = np.ascontiguousarray(np.array(probes, dtype=np.int32).reshape(max(n, 0), 3) if n else np.zeros((1, 3), np.int32))
+    out, rho = np.zeros(8), np.zeros(max(n, 1))
+    rc = _load().lbwp_oracle_diagnostics(ncomp, nx, ny, nz, _dp(m), float(threshold), n,
+                                          xyz.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), _dp(out), _dp(rho))
+    if rc != 0:
+        raise ValueError("bad arguments (probe outside the box?)")
+    return {"mass": [out[0], out[1]], "momentum": [out[2], out[3], out[4]], "rho_mean_above": out[5],
+            "count_above": int(out[6]), "rho_max": out[7], "probe_rho": [float(v) for v in rho[:n]]}

@@ -333,6 +333,39 @@ int lbwp_oracle_run(int lattice, int ncomp, int nx, int ny, int nz, double tau, 
     return 0;
 }
 
+/* ------------------------------------------------------------------------ */
+/* The paper's diagnostics: colour masses, total momentum, */
+/* <rho>_{rho > threshold} with its node count, the maximum density, and the */
+/* densities at probe sites; "rho" = density of the first component          */
+/* (its field ranges from 0 to 1).  out[8] = massA, massB,     */
+/* jx, jy, jz, mean above, count above, max.                                 */
+/* ------------------------------------------------------------------------ */
+int lbwp_oracle_diagnostics(int ncomp, int nx, int ny, int nz, const double *moments, double threshold,
+                            int nprobes, const int *probe_xyz, double *out, double *probe_rho) {
+    if ((ncomp != 1 && ncomp != 2) || nx < 1 || ny < 1 || nz < 1 || nprobes < 0) return -1;
+    const size_t n = (size_t)nx * ny * nz;
+    const int off = ncomp - 1;
+    double ma = 0.0, mb = 0.0, j[3] = {0, 0, 0}, above = 0.0, count = 0.0, mx = -1e300;
+    for (size_t p = 0; p < n; ++p) {
+        const double ra = moments[p], rb = ncomp == 2 ? moments[n + p] : 0.0;
+        ma += ra;
+        mb += rb;
+        for (int a = 0; a < 3; ++a) j[a] += (ra + rb) * moments[(off + 1 + a) * n + p];
+        if (ra > threshold) { above += ra; count += 1.0; }
+        if (ra > mx) mx = ra;
+    }
+    out[0] = ma; out[1] = mb; out[2] = j[0]; out[3] = j[1]; out[4] = j[2];
+    out[5] = count > 0.0 ? above / count : 0.0;
+    out[6] = count;
+    out[7] = mx;
+    for (int q = 0; q < nprobes; ++q) {
+        const int x = probe_xyz[3 * q], y = probe_xyz[3 * q + 1], z = probe_xyz[3 * q + 2];
+        if (x < 0 || x >= nx || y < 0 || y >= ny || z < 0 || z >= nz) return -1;
+        probe_rho[q] = moments[((size_t)z * ny + y) * nx + x];
+    }
+    return 0;
+}
+
 int lbwp_oracle_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

@@ -11,6 +11,7 @@
 #include "../../include/lbwp.h"
 #include "lbwp_common.cuh"
 #include "lbwp_convert.cuh"
+#include "lbwp_diag.cuh"
 #include "lbwp_gather.cuh"
 #include "lbwp_march.cuh"
 #include "lbwp_pop.cuh"
@@ -104,6 +105,7 @@ struct lbwp_ctx {
     bool owns = false;
     void* grad = nullptr;     // ncomp==2: colour gradient scratch, 3 fields
     void* staging = nullptr;  // dense external-layout device buffer for host <-> device I/O
+    void* diag = nullptr;     // lbwp_diagnostics: block partials, probe coordinates, results
     int cur = 0;
     int64_t steps = 0;
     cudaStream_t stream = nullptr;
@@ -501,6 +503,49 @@ int lbwp_moments(lbwp_ctx* c, void* dst, int dst_on_device) {
     return LBWP_OK;
 }
 
+int lbwp_diagnostics(lbwp_ctx* c, double threshold, int nprobes, const int32_t* probe_xyz, lbwp_diag* out, double* probe_rho) {
+    if (!c || !out || nprobes < 0 || nprobes > 4096 || (nprobes > 0 && (!probe_xyz || !probe_rho)))
+        return fail(LBWP_EINVAL, "lbwp_diagnostics: NULL argument or nprobes outside [0, 4096]");
+    for (int p = 0; p < nprobes; ++p)
+        if (probe_xyz[3 * p] < 0 || probe_xyz[3 * p] >= c->L.nx || probe_xyz[3 * p + 1] < 0 || probe_xyz[3 * p + 1] >= c->L.ny ||
+            probe_xyz[3 * p + 2] < 0 || probe_xyz[3 * p + 2] >= c->L.nz)
+            return fail(LBWP_EINVAL, "lbwp_diagnostics: probe %d lies outside the box", p);
+    DeviceGuard guard(c->P.device);
+    if (!guard.ok) return fail(LBWP_ECUDA, "cudaSetDevice(%d) failed", c->P.device);
+    if (!c->staging) CU(cudaMalloc(&c->staging, dense_bytes(c)));
+    constexpr int NP = lbwp::DIAG_NSUM + 1;
+    const size_t partial_bytes = (size_t)lbwp::DIAG_BLOCKS * NP * sizeof(double), probe_bytes = 4096 * 3 * sizeof(int),
+                 out_bytes = (NP + 4096) * sizeof(double);
+    if (!c->diag) CU(cudaMalloc(&c->diag, partial_bytes + probe_bytes + out_bytes));
+    double* partial = (double*)c->diag;
+    int* dprobes = (int*)((char*)c->diag + partial_bytes);
+    double* dout = (double*)((char*)c->diag + partial_bytes + probe_bytes);
+    int rc = c->export_dense(c->staging);   // the current moments, dense external layout
+    if (rc) return rc;
+    if (nprobes) CU(cudaMemcpyAsync(dprobes, probe_xyz, (size_t)nprobes * 3 * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    const long long n = (long long)c->L.nx * c->L.ny * c->L.nz;
+    if (c->P.dtype == LBWP_F32) {
+        if (c->P.ncomp == 1) lbwp::k_diag_partial<float, 1><<<lbwp::DIAG_BLOCKS, lbwp::DIAG_THREADS, 0, c->stream>>>((const float*)c->staging, n, threshold, partial);
+        else lbwp::k_diag_partial<float, 2><<<lbwp::DIAG_BLOCKS, lbwp::DIAG_THREADS, 0, c->stream>>>((const float*)c->staging, n, threshold, partial);
+        lbwp::k_diag_final<float><<<1, 128, 0, c->stream>>>(partial, lbwp::DIAG_BLOCKS, (const float*)c->staging, c->L.nx, c->L.ny, c->L.nz, dprobes, nprobes, dout);
+    } else {
+        if (c->P.ncomp == 1) lbwp::k_diag_partial<double, 1><<<lbwp::DIAG_BLOCKS, lbwp::DIAG_THREADS, 0, c->stream>>>((const double*)c->staging, n, threshold, partial);
+        else lbwp::k_diag_partial<double, 2><<<lbwp::DIAG_BLOCKS, lbwp::DIAG_THREADS, 0, c->stream>>>((const double*)c->staging, n, threshold, partial);
+        lbwp::k_diag_final<double><<<1, 128, 0, c->stream>>>(partial, lbwp::DIAG_BLOCKS, (const double*)c->staging, c->L.nx, c->L.ny, c->L.nz, dprobes, nprobes, dout);
+    }
+    CU(cudaGetLastError());
+    double h[NP + 4096];
+    CU(cudaMemcpyAsync(h, dout, (size_t)(NP + nprobes) * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    out->mass[0] = h[0]; out->mass[1] = h[1];
+    out->momentum[0] = h[2]; out->momentum[1] = h[3]; out->momentum[2] = h[4];
+    out->count_above = (int64_t)(h[6] + 0.5);
+    out->rho_mean_above = h[6] > 0.0 ? h[5] / h[6] : 0.0;
+    out->rho_max = h[lbwp::DIAG_NSUM];
+    for (int p = 0; p < nprobes; ++p) probe_rho[p] = h[NP + p];
+    return LBWP_OK;
+}
+
 int lbwp_set_moments(lbwp_ctx* c, const void* moments, int on_device) {
     if (!c) return fail(LBWP_EINVAL, "ctx is NULL");
     DeviceGuard guard(c->P.device);
@@ -528,6 +573,7 @@ int lbwp_destroy(lbwp_ctx* c) {
             if (c->buf[k]) cudaFree(c->buf[k]);
     if (c->grad) cudaFree(c->grad);
     if (c->staging) cudaFree(c->staging);
+    if (c->diag) cudaFree(c->diag);
     delete c;
     return LBWP_OK;
 }

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_PKG, "liblbwp.so")
 LBWP_F32, LBWP_F64 = 0, 1
 LBWP_MOMENTS, LBWP_POPULATIONS = 0, 1
 KERNELS = {"auto": 0, "gather": 1, "march": 2, "tma": 3, "tma_split": 4}
-EXPORTS = ["lbwp_state_bytes", "lbwp_num_moments", "lbwp_init", "lbwp_step", "lbwp_moments",
+EXPORTS = ["lbwp_state_bytes", "lbwp_num_moments", "lbwp_init", "lbwp_step", "lbwp_moments", "lbwp_diagnostics",
            "lbwp_set_moments", "lbwp_steps_done", "lbwp_launches_per_step", "lbwp_kernel_name",
            "lbwp_sync", "lbwp_destroy", "lbwp_last_error"]
 
@@ -36,6 +36,11 @@ class Params(ctypes.Structure):
                 ("nx", ctypes.c_int32), ("ny", ctypes.c_int32), ("nz", ctypes.c_int32),
                 ("device", ctypes.c_int32), ("tau", ctypes.c_double), ("A", ctypes.c_double),
                 ("beta", ctypes.c_double), ("stream", ctypes.c_void_p), ("buf", ctypes.c_void_p * 2)]
+
+
+class Diag(ctypes.Structure):
+    _fields_ = [("mass", ctypes.c_double * 2), ("momentum", ctypes.c_double * 3), ("rho_mean_above", ctypes.c_double),
+                ("rho_max", ctypes.c_double), ("count_above", ctypes.c_int64)]
 
 
 _lib = None
@@ -57,6 +62,8 @@ def load():
     lib.lbwp_step.argtypes = [ctypes.c_void_p, ctypes.c_int64]
     lib.lbwp_moments.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]
     lib.lbwp_set_moments.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]
+    lib.lbwp_diagnostics.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_int, ctypes.POINTER(ctypes.c_int32),
+                                     ctypes.POINTER(Diag), ctypes.POINTER(ctypes.c_double)]
     lib.lbwp_steps_done.argtypes, lib.lbwp_steps_done.restype = [ctypes.c_void_p], ctypes.c_int64
     lib.lbwp_launches_per_step.argtypes = [ctypes.c_void_p]
     lib.lbwp_kernel_name.argtypes, lib.lbwp_kernel_name.restype = [ctypes.c_void_p], ctypes.c_char_p
@@ -178,6 +185,17 @@ class Lbwp:
         else:
             _check(load().lbwp_moments(self._ctx, ctypes.c_void_p(out.data_ptr()), 0))
         return out
+
+    def diagnostics(self, threshold=0.5, probes=()):
+        """lbwp_diagnostics: dict of the paper's diagnostics of the current state; probes = [(x, y, z), ...]."""
+        n = len(probes)
+        xyz = (ctypes.c_int32 * (3 * max(n, 1)))(*[int(v) for p in probes for v in p])
+        rho = (ctypes.c_double * max(n, 1))()
+        d = Diag()
+        _check(load().lbwp_diagnostics(self._ctx, float(threshold), n, xyz if n else None, ctypes.byref(d), rho if n else None))
+        return {"mass": [d.mass[0], d.mass[1]], "momentum": [d.momentum[0], d.momentum[1], d.momentum[2]],
+                "rho_mean_above": d.rho_mean_above, "count_above": int(d.count_above), "rho_max": d.rho_max,
+                "probe_rho": [rho[i] for i in range(n)]}
 
     def sync(self):
         _check(load().lbwp_sync(self._ctx))

@@ -282,3 +282,44 @@ def test_invariants_512(lbwp):
     assert abs(px1 - px0) < 1e-7 * n ** 3 * 0.01
     # Taylor-Green decay exp(-2 nu k^2 t), nu = cs^2 (tau - 1/2) = 0.1
     assert abs(amp / 0.01 - np.exp(-2 * 0.1 * k * k * 20)) < 1e-4
+
+
+# ---- lbwp_diagnostics: the fused reduction against the oracle's, after a few steps;
+#      masses / momentum / mean to the rounding of the state, probe densities element-wise, node count exactly up to
+#      the nodes whose density sits within rounding of the threshold -------------------------------------------------
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("scheme", ["moments", "populations"])
+def test_diagnostics(lbwp, oracle, dtype, scheme):
+    cfg = wl.config3(64)
+    m0 = wl.as_dtype(cfg["moments"], dtype)
+    probes = [(16, 32, 32), (32, 32, 32), (63, 0, 5)]
+    kw = dict(lattice=27, ncomp=2, tau=0.9, A=0.01, beta=0.7)
+    with lbwp.Lbwp(m0, dtype=dtype, scheme=scheme, **kw) as sim:
+        sim.step(20)
+        got = sim.diagnostics(0.5, probes)
+        state = sim.moments_host()
+    ref = (oracle.pop_run if scheme == "populations" else oracle.run)(m0, nsteps=20, **kw)
+    want = oracle.diagnostics(ref, ncomp=2, threshold=0.5, probes=probes)
+    tol = TOL[dtype]
+    n = 64 ** 3
+    for k in (0, 1):
+        assert abs(got["mass"][k] - want["mass"][k]) <= tol * want["mass"][k]
+    assert np.abs(np.array(got["momentum"]) - want["momentum"]).max() <= tol * n * 0.05
+    assert abs(got["rho_mean_above"] - want["rho_mean_above"]) <= 10 * tol
+    assert abs(got["rho_max"] - want["rho_max"]) <= 10 * tol
+    assert np.abs(np.array(got["probe_rho"]) - want["probe_rho"]).max() <= 10 * tol
+    near = int((np.abs(ref[0] - 0.5) < 1e-4).sum())                      # nodes that rounding may move across 0.5
+    assert abs(got["count_above"] - want["count_above"]) <= near
+    # and it is exactly the reduction of what lbwp_moments returns
+    own = oracle.diagnostics(state, ncomp=2, threshold=0.5, probes=probes)
+    assert got["count_above"] == own["count_above"] and got["probe_rho"] == own["probe_rho"]
+    assert abs(got["mass"][0] - own["mass"][0]) <= 1e-9 * own["mass"][0]
+
+
+def test_diagnostics_errors(lbwp):
+    m0 = wl.as_dtype(wl.config1()["moments"], "f64")
+    with lbwp.Lbwp(m0, dtype="f64", tau=0.8) as sim:
+        d = sim.diagnostics(0.5)
+        assert d["count_above"] == 32 ** 3 and abs(d["rho_mean_above"] - 1.0) < 1e-15 and d["mass"][1] == 0.0
+        with pytest.raises(lbwp.LbwpError):
+            sim.diagnostics(0.5, [(32, 0, 0)])

@@ -135,3 +135,33 @@ def test_c8_threshold_bracket(oracle):
     u10, u30 = res[1e-10][1], res[1e-30][1]
     assert u10 < 2e-4 and u30 < 4e-4                                            # spurious currents: the part that moves
     print(f"C8 bracket: sigma {s10:.6e} vs {s30:.6e}; max|u| {u10:.3e} (1e-10) vs {u30:.3e} (1e-30)")
+
+
+# ---- the paper's diagnostics as the oracle computes them: closed-form cases ----------------------
+def test_diagnostics_closed_forms(oracle):
+    nz, ny, nx = 6, 7, 8
+    ra = np.full((nz, ny, nx), 0.125)                   # exactly representable values: the sums below are exact
+    ra[1:4, 2:5, 3:7] = 1.0                             # a 3 x 3 x 4 block of dense phase
+    u = [np.full((nz, ny, nx), v) for v in (0.25, -0.5, 0.0)]
+    m = wl.pack2(ra, 1.0 - ra, u)
+    d = oracle.diagnostics(m, ncomp=2, threshold=0.5, probes=[(3, 2, 1), (0, 0, 0), (7, 6, 5)])
+    n, vol = nz * ny * nx, 3 * 3 * 4
+    assert d["count_above"] == vol and d["rho_mean_above"] == 1.0 and d["rho_max"] == 1.0
+    assert d["mass"] == [vol + 0.125 * (n - vol), n - (vol + 0.125 * (n - vol))]
+    assert d["momentum"] == [0.25 * n, -0.5 * n, 0.0]   # rho = 1 everywhere
+    assert d["probe_rho"] == [1.0, 0.125, 0.125]
+    # single component: "density" is rho itself; nothing above the threshold gives mean 0
+    m1 = wl.pack1(np.full((nz, ny, nx), 0.25), u)
+    d1 = oracle.diagnostics(m1, ncomp=1, threshold=0.5)
+    assert d1["count_above"] == 0 and d1["rho_mean_above"] == 0.0 and d1["mass"] == [0.25 * n, 0.0]
+    with pytest.raises(ValueError):
+        oracle.diagnostics(m, ncomp=2, probes=[(8, 0, 0)])
+
+
+# the masses and the momentum it reports are the conserved sums of Eq. 1-2 over the periodic box
+def test_diagnostics_follow_conservation(oracle):
+    m = _droplet_state()
+    d0 = oracle.diagnostics(m, ncomp=2)
+    d1 = oracle.diagnostics(oracle.run(m, lattice=27, ncomp=2, tau=1.0, nsteps=5, A=0.01, beta=0.7), ncomp=2)
+    assert np.allclose(d0["mass"], d1["mass"], rtol=0, atol=1e-10)
+    assert np.allclose(d0["momentum"], d1["momentum"], rtol=0, atol=1e-11)
