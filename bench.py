@@ -14,8 +14,9 @@ The same line carries `sizes` (256^3 and 512^3, fp32 and fp64: MLUPS and the HBM
 asks), `footprint` (bytes per node and total GB with and without populations, from lbwp_state_bytes of both
 schemes) and `cpu_baseline` (the oracle on the host cores: all cores and single thread, 128^3).
 
-N > 1 (`--gpus N` under torchrun): every rank advances its own box ("replicas only" for the headline number,
-DESIGN.md); value = all ranks' node updates / max-over-ranks device time; scaling = weak.
+N > 1 (`--gpus N` under torchrun): ONE periodic box of n x n x (n N) nodes, decomposed into z slabs of n planes per
+rank (weak scaling), halo planes exchanged with the z neighbours after every step (NCCL send/recv; slabs.py);
+value = all owned node updates / max-over-ranks device time.  (The population scheme runs as replicas.)
 --impl reference: times the CPU oracle (oracle/, plain C fp64) on a bounded sample of the workload.
 """
 from __future__ import annotations
@@ -264,9 +265,25 @@ def main():
 
     peak, peak_src = measured_peak()
     nodes = a.n ** 3
-    sim, m0 = make_sim(a)
+    slab = None
+    if world > 1 and a.scheme == "moments":
+        # one periodic box of n x n x (n * world) nodes, z-slab decomposed: every rank owns n planes (weak scaling) and
+        # exchanges halo planes with its z neighbours after every step (paper_2301_01622_b200/slabs.py).  The global
+        # field is the n^3 recipe repeated along z, so each rank's halo-extended slab is cut from its own copy.
+        from paper_2301_01622_b200 import slabs
+        cfg = wl.sweep_case(a.n, a.lattice, a.ncomp, a.dtype)
+        halo = slabs.halo_width(a.ncomp)
+        m0 = wl.as_dtype(cfg["moments"], a.dtype)
+        m0 = np.ascontiguousarray(m0[:, np.arange(-halo, a.n + halo) % a.n])
+        slab = slabs.SlabLbwp(m0, world=world, rank=rank, lattice=a.lattice, dtype=a.dtype, ncomp=a.ncomp, tau=cfg["tau"],
+                              A=cfg["A"], beta=cfg["beta"], kernel=a.kernel, device=local)
+        sim = slab.sim
+        stepper = slab
+    else:
+        sim, m0 = make_sim(a)
+        stepper = sim
     kname, lps, state_bytes = sim.kernel_name, sim.launches_per_step, sim.state_bytes
-    sim.step(max(3, a.warmup))
+    stepper.step(max(3, a.warmup))
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
@@ -274,7 +291,7 @@ def main():
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     ev0.record()
-    sim.step(a.steps)          # exactly K steps, K * launches_per_step kernel launches, nothing else in the region
+    stepper.step(a.steps)      # exactly K steps: K * launches_per_step kernel launches (N > 1: plus the halo exchange)
     ev1.record()
     barrier()
     clocks = sampler.stop()
@@ -301,7 +318,7 @@ def main():
         barrier()
         dt = max_over_ranks(time.perf_counter() - t0, world, "cuda")
         nbytes = h_in.numel() * h_in.element_size()
-        e2e = {"value": nodes * a.e2e_steps * world / dt / 1e6, "unit": METRIC, "h2d_bytes_per_step": nbytes,
+        e2e = {"value": m0.shape[1] * a.n * a.n * a.e2e_steps * world / dt / 1e6, "unit": METRIC, "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes, "steps": a.e2e_steps,
                "what": "lbwp_set_moments(host) + lbwp_step(1) + lbwp_moments(host) per step, pinned host buffers"}
         del h_in, h_out
@@ -353,7 +370,8 @@ def main():
         "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": a.dtype, "data": "synthetic",
         "config": {"workload": workload_name(a), "kernel": kname, "grid": [a.n] * 3, "l2": "state 2 x %.2f GB >> 126 MB L2, no flush needed" % (state_bytes / 1e9) if state_bytes > 4e8 else "state partly L2-resident (reported as is)",
-                   "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "parallelism": ("z-slabs of one %d x %d x %d box, %d-plane halo exchange per step (NCCL send/recv)" % (a.n, a.n, a.n * world, slab.halo)
+                                   if slab is not None else "replicas only" if world > 1 else "1 GPU"),
                    "bytes_per_node_state": state_bytes * 2 / nodes},
         "clocks": clocks,
         "e2e": e2e,

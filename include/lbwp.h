@@ -128,6 +128,22 @@ typedef struct lbwp_diag {
 int lbwp_diagnostics(lbwp_ctx *ctx, double threshold, int nprobes, const int32_t *probe_xyz, lbwp_diag *out,
                      double *probe_rho);
 
+/* z-slab decomposition over several GPUs (the paper's motivation are grids of billions of nodes,
+ * PAPER.md:163-167).  A rank's context is an ordinary periodic box whose first and last H planes are HALO planes:
+ * copies of the neighbouring ranks' boundary planes (H = 1; H = 2 for ncomp == 2 moments, whose colour gradient
+ * reaches two planes).  One step of the decomposed box = lbwp_step(ctx, 1) on every rank, then every rank packs its
+ * H lowest and H highest OWNED planes of the new state, sends them to its z neighbours (NCCL send/recv, or a peer
+ * copy) and unpacks what it receives into its halo planes.  The planes the step computed INTO the halo are garbage
+ * (the box wrapped onto itself there) and are overwritten by the unpack.  The packed format is the library's private
+ * state layout: only contexts with identical params and step count may exchange it.
+ *   lbwp_halo_bytes   bytes of nplanes packed planes (0 on error)
+ *   lbwp_halo_pack    planes [z0, z0 + nplanes) of the CURRENT state -> dst (DEVICE pointer), asynchronous on the stream
+ *   lbwp_halo_unpack  src (DEVICE pointer) -> planes [z0, z0 + nplanes) of the current state, asynchronous
+ * LBWP_EINVAL if the plane range leaves the box. */
+size_t lbwp_halo_bytes(const lbwp_ctx *ctx, int nplanes);
+int lbwp_halo_pack(lbwp_ctx *ctx, int z0, int nplanes, void *dst);
+int lbwp_halo_unpack(lbwp_ctx *ctx, int z0, int nplanes, const void *src);
+
 /* Replace the state by new moments (same conventions as lbwp_init); step counter -> 0. */
 int lbwp_set_moments(lbwp_ctx *ctx, const void *moments, int moments_on_device);
 

@@ -116,6 +116,10 @@ struct lbwp_ctx {
     virtual int step_once() = 0;
     virtual int import_dense(const void* dev_ext) = 0;
     virtual int export_dense(void* dev_ext) = 0;
+    // geometry of z planes in the state buffers, in elements: field stride, plane stride, offset of logical plane 0,
+    // number of state fields; and the buffer that holds the CURRENT state (halo exchange, lbwp_halo_*)
+    virtual void plane_geometry(long long* field, long long* plane, long long* z0off, int* nf) const = 0;
+    virtual void* state_buffer() const { return buf[cur]; }
 };
 
 namespace {
@@ -200,6 +204,9 @@ struct Ctx final : lbwp_ctx {
         return LBWP_OK;
     }
 
+    void plane_geometry(long long* field, long long* plane, long long* z0off, int* nf) const override {
+        *field = L.field; *plane = L.plane; *z0off = L.plane; *nf = nfields;   // one ghost plane below logical plane 0
+    }
     int export_dense(void* ext) override {
         const dim3 b(32, 8, 1), g = node_grid(L, b);
         if (P.scheme == LBWP_POPULATIONS) {
@@ -251,6 +258,9 @@ struct TmaCtx final : lbwp_ctx {
         CU(cudaGetLastError());
         return LBWP_OK;
     }
+    void plane_geometry(long long* field, long long* plane, long long* z0off, int* nf) const override {
+        *field = X.field; *plane = X.plane; *z0off = 0; *nf = 10;
+    }
     int export_dense(void* ext) override {
         if (steps == 0) {
             const dim3 b(32, 8, 1), g((X.nx + 31) / 32, (X.ny + 7) / 8, X.nz);
@@ -292,6 +302,10 @@ struct Tma2Ctx final : lbwp_ctx {
         CU(cudaGetLastError());
         return LBWP_OK;
     }
+    void plane_geometry(long long* field, long long* plane, long long* z0off, int* nf) const override {
+        *field = X.field; *plane = X.plane; *z0off = 0; *nf = 12;
+    }
+    void* state_buffer() const override { return buf[1]; }   // R; buf[0] is the scratch of the collide pass
     int export_dense(void* ext) override {
         const dim3 b(32, 8, 1), g((X.nx + 31) / 32, (X.ny + 7) / 8, X.nz);
         lbwp::k_tma2_export<T><<<g, b, 0, stream>>>(X, (const T*)buf[1], (T*)ext);
@@ -329,6 +343,9 @@ struct Tma2gCtx final : lbwp_ctx {
         int rc = planp->import_state(ext, buf[0], buf[1], 1.0 / P.tau, stream);
         if (rc) return fail(LBWP_ECUDA, "import launch: %s", cudaGetErrorString((cudaError_t)rc));
         return LBWP_OK;
+    }
+    void plane_geometry(long long* field, long long* plane, long long* z0off, int* nf) const override {
+        *field = X.field; *plane = X.plane; *z0off = 0; *nf = 11;
     }
     int export_dense(void* ext) override {
         if (steps == 0) {
@@ -545,6 +562,35 @@ int lbwp_diagnostics(lbwp_ctx* c, double threshold, int nprobes, const int32_t* 
     for (int p = 0; p < nprobes; ++p) probe_rho[p] = h[NP + p];
     return LBWP_OK;
 }
+
+namespace {
+int halo_copy(lbwp_ctx* c, int z0, int nplanes, void* packed, bool pack) {
+    if (!c || !packed) return fail(LBWP_EINVAL, "lbwp_halo_*: NULL argument");
+    if (c->P.scheme != LBWP_MOMENTS) return fail(LBWP_EUNSUPPORTED, "lbwp_halo_*: moments scheme only");
+    if (nplanes < 1 || z0 < 0 || z0 + nplanes > c->L.nz) return fail(LBWP_EINVAL, "lbwp_halo_*: planes [%d, %d) leave the box", z0, z0 + nplanes);
+    DeviceGuard guard(c->P.device);
+    if (!guard.ok) return fail(LBWP_ECUDA, "cudaSetDevice(%d) failed", c->P.device);
+    long long field, plane, z0off;
+    int nf;
+    c->plane_geometry(&field, &plane, &z0off, &nf);
+    // nf rows (one per state field) of nplanes contiguous planes each: one strided 2-D copy
+    char* state = (char*)c->state_buffer() + (size_t)(z0off + (long long)z0 * plane) * c->esize;
+    const size_t width = (size_t)nplanes * plane * c->esize, pitch = (size_t)field * c->esize;
+    if (pack) CU(cudaMemcpy2DAsync(packed, width, state, pitch, width, nf, cudaMemcpyDeviceToDevice, c->stream));
+    else CU(cudaMemcpy2DAsync(state, pitch, packed, width, width, nf, cudaMemcpyDeviceToDevice, c->stream));
+    return LBWP_OK;
+}
+}  // namespace
+
+size_t lbwp_halo_bytes(const lbwp_ctx* c, int nplanes) {
+    if (!c || nplanes < 1 || c->P.scheme != LBWP_MOMENTS) return 0;
+    long long field, plane, z0off;
+    int nf;
+    c->plane_geometry(&field, &plane, &z0off, &nf);
+    return (size_t)nf * nplanes * plane * c->esize;
+}
+int lbwp_halo_pack(lbwp_ctx* c, int z0, int nplanes, void* dst) { return halo_copy(c, z0, nplanes, dst, true); }
+int lbwp_halo_unpack(lbwp_ctx* c, int z0, int nplanes, const void* src) { return halo_copy(c, z0, nplanes, const_cast<void*>(src), false); }
 
 int lbwp_set_moments(lbwp_ctx* c, const void* moments, int on_device) {
     if (!c) return fail(LBWP_EINVAL, "ctx is NULL");

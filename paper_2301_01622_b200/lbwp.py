@@ -20,7 +20,7 @@ LBWP_F32, LBWP_F64 = 0, 1
 LBWP_MOMENTS, LBWP_POPULATIONS = 0, 1
 KERNELS = {"auto": 0, "gather": 1, "march": 2, "tma": 3, "tma_split": 4}
 EXPORTS = ["lbwp_state_bytes", "lbwp_num_moments", "lbwp_init", "lbwp_step", "lbwp_moments", "lbwp_diagnostics",
-           "lbwp_set_moments", "lbwp_steps_done", "lbwp_launches_per_step", "lbwp_kernel_name",
+           "lbwp_halo_bytes", "lbwp_halo_pack", "lbwp_halo_unpack", "lbwp_set_moments", "lbwp_steps_done", "lbwp_launches_per_step", "lbwp_kernel_name",
            "lbwp_sync", "lbwp_destroy", "lbwp_last_error"]
 
 
@@ -64,6 +64,9 @@ def load():
     lib.lbwp_set_moments.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]
     lib.lbwp_diagnostics.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_int, ctypes.POINTER(ctypes.c_int32),
                                      ctypes.POINTER(Diag), ctypes.POINTER(ctypes.c_double)]
+    lib.lbwp_halo_bytes.argtypes, lib.lbwp_halo_bytes.restype = [ctypes.c_void_p, ctypes.c_int], ctypes.c_size_t
+    lib.lbwp_halo_pack.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p]
+    lib.lbwp_halo_unpack.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p]
     lib.lbwp_steps_done.argtypes, lib.lbwp_steps_done.restype = [ctypes.c_void_p], ctypes.c_int64
     lib.lbwp_launches_per_step.argtypes = [ctypes.c_void_p]
     lib.lbwp_kernel_name.argtypes, lib.lbwp_kernel_name.restype = [ctypes.c_void_p], ctypes.c_char_p
@@ -196,6 +199,20 @@ class Lbwp:
         return {"mass": [d.mass[0], d.mass[1]], "momentum": [d.momentum[0], d.momentum[1], d.momentum[2]],
                 "rho_mean_above": d.rho_mean_above, "count_above": int(d.count_above), "rho_max": d.rho_max,
                 "probe_rho": [rho[i] for i in range(n)]}
+
+    def halo_bytes(self, nplanes) -> int:
+        return int(load().lbwp_halo_bytes(self._ctx, int(nplanes)))
+
+    def halo_pack(self, z0, nplanes, dst):
+        """lbwp_halo_pack into a torch uint8 CUDA tensor of halo_bytes(nplanes) bytes (asynchronous)."""
+        if dst.numel() * dst.element_size() < self.halo_bytes(nplanes) or not dst.is_cuda or not dst.is_contiguous():
+            raise ValueError("dst must be a contiguous CUDA tensor of at least halo_bytes(nplanes) bytes")
+        _check(load().lbwp_halo_pack(self._ctx, int(z0), int(nplanes), ctypes.c_void_p(dst.data_ptr())))
+
+    def halo_unpack(self, z0, nplanes, src):
+        if src.numel() * src.element_size() < self.halo_bytes(nplanes) or not src.is_cuda or not src.is_contiguous():
+            raise ValueError("src must be a contiguous CUDA tensor of at least halo_bytes(nplanes) bytes")
+        _check(load().lbwp_halo_unpack(self._ctx, int(z0), int(nplanes), ctypes.c_void_p(src.data_ptr())))
 
     def sync(self):
         _check(load().lbwp_sync(self._ctx))
