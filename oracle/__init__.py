@@ -43,6 +43,8 @@ def _load():
         lib.lbwp_oracle_run.argtypes = run_args
         lib.lbwp_oracle_pop_run.argtypes = run_args
         lib.lbwp_oracle_threads.restype = ctypes.c_int
+        lib.lbwp_oracle_reconstruct_forced.argtypes = [ctypes.c_int, dp, ctypes.c_double, dp, dp]
+        lib.lbwp_oracle_run_nc.argtypes = [ctypes.c_int] * 4 + [ctypes.c_double] * 5 + [dp, ctypes.c_int64, dp]
         lib.lbwp_oracle_diagnostics.argtypes = [ctypes.c_int] * 4 + [dp, ctypes.c_double, ctypes.c_int, ip, dp, dp]
         lib.lbwp_oracle_set_threads.argtypes, lib.lbwp_oracle_set_threads.restype = [ctypes.c_int], ctypes.c_int
         lib.lbwp_oracle_set_g2cut.argtypes = [ctypes.c_double]
@@ -139,3 +141,30 @@ def diagnostics(moments, *, ncomp: int = 1, threshold: float = 0.5, probes=()) -
         raise ValueError("bad arguments (probe outside the box?)")
     return {"mass": [out[0], out[1]], "momentum": [out[2], out[3], out[4]], "rho_mean_above": out[5],
             "count_above": int(out[6]), "rho_max": out[7], "probe_rho": [float(v) for v in rho[:n]]}
+
+
+def run_nc(moments, *, lattice: int, tau: float, nsteps: int, A: float, beta: float, A_h: float, h_c: float = 4.0,
+           return_force: bool = False):
+    """Two-component run with the near-contact repulsion of PAPER.md Eq. 10 (readings C20-C24); with return_force
+    also the force field [3,nz,ny,nx] of the last step."""
+    m = np.array(moments, dtype=np.float64, order="C", copy=True)
+    if m.ndim != 4 or m.shape[0] != 11:
+        raise ValueError("moments must have shape [11, nz, ny, nx]")
+    _, nz, ny, nx = m.shape
+    f = np.zeros((3, nz, ny, nx))
+    rc = _load().lbwp_oracle_run_nc(lattice, nx, ny, nz, float(tau), float(A), float(beta), float(A_h), float(h_c),
+                                    _dp(m), int(nsteps), _dp(f))
+    if rc != 0:
+        raise RuntimeError(f"oracle returned {rc}")
+    return (m, f) if return_force else m
+
+
+def reconstruct_forced(q: int, H10, omega: float, F3) -> np.ndarray:
+    """Eq. 8 populations of one node under a body force F (reading C24)."""
+    H = np.ascontiguousarray(H10, dtype=np.float64)
+    F = np.ascontiguousarray(F3, dtype=np.float64)
+    out = np.zeros(27, dtype=np.float64)
+    n = _load().lbwp_oracle_reconstruct_forced(q, _dp(H), float(omega), _dp(F), _dp(out))
+    if n < 0:
+        raise ValueError("lattice must be 19 or 27")
+    return out[:n].copy()

@@ -297,6 +297,169 @@ static void step_2c(const lattice_t *L, int nx, int ny, int nz, double omega, do
 }
 
 /* ------------------------------------------------------------------------ */
+/* Near-contact repulsion (Eq. 10):                          */
+/*     F_rep = - A_h[h(x)] n delta_I .                                        */
+/* The paper gives neither h(x) nor the forcing scheme (both are in its ref.  */
+/* [26]); readings C20-C24 of DESIGN.md, PARITY WITH THE PAPER'S CODE         */
+/* UNPINNED:                                                                  */
+/*  C20 delta_I = |grad phi| / 2 = |G|/2 (integrates to 1 across an interface)*/
+/*  C21 n = outward unit normal of the droplet phase = -G/|G| (phi = +1       */
+/*      inside), so F_rep = (A_h/2) G: it pushes an interface away from the   */
+/*      one it faces.                                                         */
+/*  C22 h(x), at INTERFACE nodes, |G| > G_I = 0.05 (a tenth of the peak        */
+/*      gradient 1/W of a tanh interface of width W = 2): walk from x along    */
+/*      the lattice direction c_m closest to n (largest c.n/|c|; first in      */
+/*      direction order on a tie), p_k = x + k c_m, k = 1, 2, ... while        */
+/*      k |c_m| <= h_c; the first interface node p_k whose gradient opposes    */
+/*      G (G(p_k).G(x) < 0, |G(p_k)| > G_I) is a facing interface and          */
+/*      h = k |c_m|; none: h = infinity.                                       */
+/*  C23 A_h[h] = A_h for h <= h_c, 0 beyond (one strength).     */
+/*  C24 forcing in moment space: Guo's scheme on the reconstructed            */
+/*      populations, see hprime_forced().                                     */
+/* force: 3*n doubles Fx, Fy, Fz.                                             */
+/* ------------------------------------------------------------------------ */
+#define G_I2 (0.05 * 0.05)
+static void contact_force(const lattice_t *L, int nx, int ny, int nz, const double *grad, double A_h,
+                          double h_c, double *force) {
+    const size_t n = (size_t)nx * ny * nz;
+#pragma omp parallel for schedule(static)
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) {
+                const size_t xx = ((size_t)z * ny + y) * nx + x;
+                double G[3] = {grad[xx], grad[n + xx], grad[2 * n + xx]};
+                double F[3] = {0, 0, 0};
+                const double g2 = G[0] * G[0] + G[1] * G[1] + G[2] * G[2];
+                if (g2 > G_I2 && A_h != 0.0) {
+                    int m = -1;
+                    double best = -1e300;
+                    for (int i = 0; i < L->q; ++i) { /* lattice direction closest to n = -G/|G| */
+                        const int *c = L->c[i];
+                        const int c2 = c[0] * c[0] + c[1] * c[1] + c[2] * c[2];
+                        if (c2 == 0) continue;
+                        const double cosv = -(c[0] * G[0] + c[1] * G[1] + c[2] * G[2]) / sqrt((double)c2);
+                        if (cosv > best) { best = cosv; m = i; }
+                    }
+                    const int *c = L->c[m];
+                    const double len = sqrt((double)(c[0] * c[0] + c[1] * c[1] + c[2] * c[2]));
+                    for (int k = 1; k * len <= h_c; ++k) {
+                        const size_t pp = ((size_t)wrap(z + k * c[2], nz) * ny + wrap(y + k * c[1], ny)) * nx +
+                                          wrap(x + k * c[0], nx);
+                        const double Gp[3] = {grad[pp], grad[n + pp], grad[2 * n + pp]};
+                        const double gp2 = Gp[0] * Gp[0] + Gp[1] * Gp[1] + Gp[2] * Gp[2];
+                        if (gp2 > G_I2 && Gp[0] * G[0] + Gp[1] * G[1] + Gp[2] * G[2] < 0.0) {
+                            for (int a = 0; a < 3; ++a) F[a] = 0.5 * A_h * G[a]; /* -A_h n delta_I */
+                            break;
+                        }
+                    }
+                }
+                for (int a = 0; a < 3; ++a) force[a * n + xx] = F[a];
+            }
+}
+
+/* Eq. 8 with a body force F (reading C24): Guo, Zheng and Shi's forcing on the   */
+/* reconstructed populations.  u* = u + F/(2 rho) is the velocity of the         */
+/* equilibrium; the stored first moment rho u differs from rho u* by -F/2, a     */
+/* first-order non-equilibrium part that relaxes like the second-order one;      */
+/* S_i = (1 - omega/2) w_i [ (c_i - u*)/cs^2 + (c_i.u*) c_i / cs^4 ] . F.         */
+/* Its moments: sum_i = rho, sum_i c_i = rho u + F (momentum gains F per step),  */
+/* F = 0 gives hprime().                                                         */
+static double hprime_forced(const lattice_t *L, int i, double rho, const double u[3], const double P[6],
+                            double omega, const double F[3]) {
+    const int *c = L->c[i];
+    double us[3], cu = 0.0, cF = 0.0, uF = 0.0, cdu = 0.0;
+    for (int a = 0; a < 3; ++a) us[a] = u[a] + F[a] / (2.0 * rho);
+    for (int a = 0; a < 3; ++a) {
+        cu += c[a] * us[a];
+        cF += c[a] * F[a];
+        uF += us[a] * F[a];
+        cdu += c[a] * (rho * u[a] - rho * us[a]);
+    }
+    double quu = 0.0, qneq = 0.0;
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) {
+            double q = Qiab(c, a, b);
+            double peq = rho * us[a] * us[b] + (a == b ? rho * CS2 : 0.0);
+            quu += q * us[a] * us[b];
+            qneq += q * (P[PIDX[a][b]] - peq);
+        }
+    double heq = L->w[i] * rho * (1.0 + cu / CS2 + quu);
+    double hneq = L->w[i] * (qneq + cdu / CS2);
+    double Si = (1.0 - 0.5 * omega) * L->w[i] * ((cF - uF) / CS2 + cu * cF / (CS2 * CS2));
+    return heq + (1.0 - omega) * hneq + Si;
+}
+
+/* all directions of hprime_forced for one node (pins of the forcing term) */
+int lbwp_oracle_reconstruct_forced(int lattice, const double *H10, double omega, const double *F3, double *h_out) {
+    lattice_t L;
+    if (lattice_make(lattice, &L)) return -1;
+    for (int i = 0; i < L.q; ++i) h_out[i] = hprime_forced(&L, i, H10[0], H10 + 1, H10 + 4, omega, F3);
+    return L.q;
+}
+
+/* two-component step with the near-contact force: step_2c with hprime_forced */
+static void step_2c_nc(const lattice_t *L, int nx, int ny, int nz, double omega, double A, double beta,
+                       double A_h, double h_c, const double *src, double *dst, double *grad, double *force) {
+    const size_t n = (size_t)nx * ny * nz;
+    colour_gradient(L, nx, ny, nz, src, src + n, grad);
+    contact_force(L, nx, ny, nz, grad, A_h, h_c, force);
+#pragma omp parallel for schedule(static)
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) {
+                double rA = 0.0, rB = 0.0, j[3] = {0, 0, 0}, P[6] = {0, 0, 0, 0, 0, 0};
+                for (int i = 0; i < L->q; ++i) {
+                    const int *c = L->c[i];
+                    size_t yy = ((size_t)wrap(z - c[2], nz) * ny + wrap(y - c[1], ny)) * nx +
+                                wrap(x - c[0], nx);
+                    double u[3], Pn[6], G[3], F[3];
+                    double a_ = src[yy], b_ = src[n + yy];
+                    for (int a = 0; a < 3; ++a) u[a] = src[(2 + a) * n + yy];
+                    for (int k = 0; k < 6; ++k) Pn[k] = src[(5 + k) * n + yy];
+                    for (int a = 0; a < 3; ++a) G[a] = grad[a * n + yy];
+                    for (int a = 0; a < 3; ++a) F[a] = force[a * n + yy];
+                    double hp = hprime_forced(L, i, a_ + b_, u, Pn, omega, F);
+                    double hA, hB;
+                    colour_ops(L, i, hp, a_, b_, G, A, beta, &hA, &hB);
+                    double hpp = hA + hB;
+                    rA += hA;
+                    rB += hB;
+                    for (int a = 0; a < 3; ++a) j[a] += hpp * c[a];
+                    for (int a = 0; a < 3; ++a)
+                        for (int b = a; b < 3; ++b) P[PIDX[a][b]] += hpp * c[a] * c[b];
+                }
+                size_t xx = ((size_t)z * ny + y) * nx + x;
+                dst[xx] = rA;
+                dst[n + xx] = rB;
+                for (int a = 0; a < 3; ++a) dst[(2 + a) * n + xx] = j[a] / (rA + rB);
+                for (int k = 0; k < 6; ++k) dst[(5 + k) * n + xx] = P[k];
+            }
+}
+
+/* Two-component run with the near-contact force; force_out (3*n doubles or NULL) receives the force field of the
+ * LAST step taken (diagnostic: the pins integrate it). */
+int lbwp_oracle_run_nc(int lattice, int nx, int ny, int nz, double tau, double A, double beta, double A_h,
+                       double h_c, double *moments, int64_t nsteps, double *force_out) {
+    lattice_t L;
+    if (lattice_make(lattice, &L)) return -1;
+    if (nx < 1 || ny < 1 || nz < 1 || !(tau > 0.5) || nsteps < 0 || !(h_c >= 0.0)) return -1;
+    const size_t n = (size_t)nx * ny * nz;
+    double *buf = (double *)malloc(sizeof(double) * 11 * n);
+    double *grad = (double *)malloc(sizeof(double) * 4 * n);
+    double *force = (double *)calloc(3 * n, sizeof(double));
+    if (!buf || !grad || !force) { free(buf); free(grad); free(force); return -2; }
+    double *cur = moments, *nxt = buf;
+    for (int64_t t = 0; t < nsteps; ++t) {
+        step_2c_nc(&L, nx, ny, nz, 1.0 / tau, A, beta, A_h, h_c, cur, nxt, grad, force);
+        double *tmp = cur; cur = nxt; nxt = tmp;
+    }
+    if (cur != moments) memcpy(moments, cur, sizeof(double) * 11 * n);
+    if (force_out) memcpy(force_out, force, sizeof(double) * 3 * n);
+    free(buf); free(grad); free(force);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------ */
 /* Public entry: advance `moments` (M*n doubles, layout above) by nsteps,    */
 /* in place, with internal ping-pong ("Flip-Flop").              */
 /* omega = 1/tau (reading C3).  Returns 0, or -1 on bad arguments / -2 on    */
