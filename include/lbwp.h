@@ -76,6 +76,13 @@ typedef struct lbwp_params {
     void *buf[2];        /* optional caller-owned DEVICE buffers, each >= lbwp_state_bytes() bytes and
                             256-byte aligned (e.g. a torch tensor's data_ptr); must outlive the ctx.
                             NULL, NULL => the library allocates and frees them. */
+    double A_h;          /* ncomp == 2, moments scheme: strength of the near-contact repulsion
+                            F_rep = -A_h[h(x)] n delta_I (Eq. 10; readings C20-C24 of DESIGN.md:
+                            delta_I = |grad phi|/2, n the outward normal, A_h[h] = A_h for h <= h_c and 0 beyond,
+                            Guo forcing).  0 = off (BASELINE's configs).  Non-zero selects the generic kernel
+                            (three launches per step: gradient, contact search, step); LBWP_EUNSUPPORTED with
+                            LBWP_KERNEL_TMA / TMA_SPLIT / MARCH. */
+    double h_c;          /* cut-off distance of the near-contact force in lattice units (> 0 when A_h != 0) */
 } lbwp_params;
 
 /* Bytes of ONE internal state buffer (ghost layers and padding included) for these

@@ -62,6 +62,8 @@ bool params_ok(const lbwp_params* p) {
     if (p->nz > 65535 || (p->ny + 7) / 8 > 65535) return false;   // the pointwise kernels put z (and y / 8) in gridDim.z (.y)
     if (!(p->tau > 0.5)) return false;  // also rejects NaN
     if ((p->buf[0] == nullptr) != (p->buf[1] == nullptr)) return false;
+    if (p->A_h != 0.0 && !(p->ncomp == 2 && p->scheme == LBWP_MOMENTS && p->h_c > 0.0)) return false;   // also rejects NaN h_c
+    if (p->A_h != p->A_h) return false;
     return true;
 }
 
@@ -85,6 +87,8 @@ bool tma2_fused(const lbwp_params* p) { return p->ncomp == 2 && p->kernel != LBW
 
 // kernel variant a context with these params runs (LBWP_KERNEL_AUTO resolved); 0 if not built
 int choose_variant(const lbwp_params* p) {
+    if (p->A_h != 0.0)   // near-contact force: built into the generic kernels only
+        return (p->kernel == LBWP_KERNEL_AUTO || p->kernel == LBWP_KERNEL_GATHER) ? LBWP_KERNEL_GATHER : 0;
     const bool march_ok = p->scheme == LBWP_MOMENTS && p->ncomp == 1 && p->lattice == 27;
     switch (p->kernel) {
         case LBWP_KERNEL_AUTO: return tma_eligible(p) ? LBWP_KERNEL_TMA : march_ok ? LBWP_KERNEL_MARCH : LBWP_KERNEL_GATHER;
@@ -137,6 +141,11 @@ struct Ctx final : lbwp_ctx {
         s.omega = T(1.0 / P.tau);
         s.A = T(P.A);
         s.beta = T(P.beta);
+        if (P.A_h != 0.0) {
+            s.force = (const T*)grad + 3 * L.field;   // scratch: 3 gradient + 3 force fields
+            s.A_h = T(P.A_h);
+            s.h_c = T(P.h_c);
+        }
         return s;
     }
 
@@ -145,6 +154,11 @@ struct Ctx final : lbwp_ctx {
         const dim3 b(32, 8, 1), g = node_grid(L, b);
         if (NC == 2) lbwp::k_colour_gradient<T, Q><<<g, b, 0, stream>>>(s, (T*)grad);
         if (NC == 1 && Q == 27 && variant == LBWP_KERNEL_MARCH) return lbwp::launch_march27<T>(s, stream);
+        if (NC == 2 && s.force) {
+            lbwp::k_near_contact<T, Q><<<g, b, 0, stream>>>(s, (const T*)grad, (T*)grad + 3 * L.field);
+            lbwp::k_step_gather<T, Q, 2, 1><<<g, b, 0, stream>>>(s);
+            return 0;
+        }
         lbwp::k_step_gather<T, Q, NC><<<g, b, 0, stream>>>(s);
         return 0;
     }
@@ -396,12 +410,12 @@ int lbwp_num_moments(const lbwp_params* p) { return params_ok(p) ? num_moments(p
 
 int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, lbwp_ctx** out) {
     if (!out) return fail(LBWP_EINVAL, "out is NULL");
-    if (!params_ok(p)) return fail(LBWP_EINVAL, "invalid lbwp_params (lattice 19|27, dtype, ncomp 1|2, sizes >= 1, tau > 0.5, struct_size)");
+    if (!params_ok(p)) return fail(LBWP_EINVAL, "invalid lbwp_params (lattice 19|27, dtype, ncomp 1|2, sizes >= 1, tau > 0.5, A_h only with ncomp 2 moments and h_c > 0, struct_size)");
     if (!moments) return fail(LBWP_EINVAL, "moments is NULL");
     const int variant = choose_variant(p);
     if (variant == 0)
         return fail(LBWP_EUNSUPPORTED, "kernel %d is not built for this combination (MARCH: D3Q27 single-component moments; TMA: moments "
-                    "scheme with nx %% 64 (fp32) or 32 (fp64) == 0 and ny %% 8 == 0; TMA_SPLIT: two-component only)", p->kernel);
+                    "scheme with nx %% 64 (fp32) or 32 (fp64) == 0 and ny %% 8 == 0; TMA_SPLIT: two-component only; A_h != 0: AUTO or GATHER)", p->kernel);
     int ndev = 0;
     CU(cudaGetDeviceCount(&ndev));
     if (p->device < 0 || p->device >= ndev) return fail(LBWP_EINVAL, "device %d out of range (%d devices)", p->device, ndev);
@@ -448,9 +462,10 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
         }
     }
     if (p->scheme == LBWP_MOMENTS && p->ncomp == 2 && variant != LBWP_KERNEL_TMA) {
-        cudaError_t e = cudaMalloc(&c->grad, (size_t)3 * c->L.field * c->esize);
+        const bool nc = p->A_h != 0.0;
+        cudaError_t e = cudaMalloc(&c->grad, (size_t)(nc ? 6 : 3) * c->L.field * c->esize);
         if (e != cudaSuccess) return bail(fail(LBWP_ENOMEM, "cudaMalloc(grad): %s", cudaGetErrorString(e)));
-        c->launches_per_step = 2;
+        c->launches_per_step = nc ? 3 : 2;
     }
     if (p->scheme == LBWP_POPULATIONS && p->ncomp == 2) {
         const size_t gb = (size_t)5 * c->L.field * c->esize;  // 3 gradient + 2 density fields

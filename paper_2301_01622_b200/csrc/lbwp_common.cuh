@@ -55,6 +55,8 @@ struct StepParams {
     const T* __restrict__ grad;  // ncomp==2: 3 fields Gx,Gy,Gz (same layout), else nullptr
     T omega;                     // 1/tau            (reading C3)
     T A, beta;                   // colour gradient  (reading C6)
+    const T* __restrict__ force = nullptr;   // near-contact force Fx, Fy, Fz (same layout), or nullptr (readings C20-C24)
+    T A_h = T(0), h_c = T(0);    // its strength and cut-off distance (Eq. 10)
 };
 
 // Store v at interior node (x,y,z) of one field and at each of its periodic ghost

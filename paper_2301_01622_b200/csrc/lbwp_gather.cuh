@@ -67,7 +67,9 @@ struct Acc {
 
 // One direction of the pull: read the moments at y = x - c, collide there (Eq. 8),
 // add the arriving population to the node's moment sums (Eq. 9, Eq. 1-3).
-template <typename T, int Q, int NC, int CX, int CY, int CZ>
+// NF = 1: with the near-contact body force F(y) (reading C24, Guo forcing on the reconstructed populations):
+//   u* = u + F/(2 rho) in the quadratic terms, j + F in the linear term, S += (1 - omega/2)(u* F + F u*).
+template <typename T, int Q, int NC, int CX, int CY, int CZ, int NF = 0>
 __device__ __forceinline__ void pull_dir(const StepParams<T>& p, long long xc, Acc<T>& a) {
     constexpr int N2 = CX * CX + CY * CY + CZ * CZ;
     if (Q == 19 && N2 == 3) return;
@@ -84,8 +86,26 @@ __device__ __forceinline__ void pull_dir(const StepParams<T>& p, long long xc, A
         // colour gradient (reading C6): perturbation folded into (da, S), rest-population
         // term E0, then recolouring of the arriving population.
         const T rhoA = s[y], drho = s[F + y];
-        SNode<T> n = collide_sform<T>(drho, s[2 * F + y], s[3 * F + y], s[4 * F + y], s[5 * F + y], s[6 * F + y],
+        T ux = s[2 * F + y], uy = s[3 * F + y], uz = s[4 * F + y];
+        T fx = T(0), fy = T(0), fz = T(0);
+        if (NF) {
+            fx = p.force[y]; fy = p.force[F + y]; fz = p.force[2 * F + y];
+            const T hr = T(0.5) / (T(1) + drho);
+            ux += hr * fx; uy += hr * fy; uz += hr * fz;          // u*
+        }
+        SNode<T> n = collide_sform<T>(drho, ux, uy, uz, s[5 * F + y], s[6 * F + y],
                                       s[7 * F + y], s[8 * F + y], s[9 * F + y], s[10 * F + y], p.omega);
+        if (NF) {
+            // J = 3 (j + F) (collide_sform gave 3 rho u* = 3 (j + F/2)); S-form of (1 - omega/2)(u* F + F u*)
+            n.Jx += T(1.5) * fx; n.Jy += T(1.5) * fy; n.Jz += T(1.5) * fz;
+            const T k = T(1) - T(0.5) * p.omega;
+            const T dxx = T(2) * k * ux * fx, dyy = T(2) * k * uy * fy, dzz = T(2) * k * uz * fz;
+            n.da -= T(1.5) * (dxx + dyy + dzz);
+            n.Sxx += T(4.5) * dxx; n.Syy += T(4.5) * dyy; n.Szz += T(4.5) * dzz;
+            n.Sxy += T(9) * k * (ux * fy + uy * fx);
+            n.Sxz += T(9) * k * (ux * fz + uz * fx);
+            n.Syz += T(9) * k * (uy * fz + uz * fy);
+        }
         const T Gx = p.grad[y], Gy = p.grad[F + y], Gz = p.grad[2 * F + y];
         const T g2 = Gx * Gx + Gy * Gy + Gz * Gz;
         const T ig = g2 > T(1e-10) ? rsqrt_t<T>(g2) : T(0);  // reading C8: |G| <= 1e-5 -> n = 0
@@ -126,7 +146,7 @@ __device__ __forceinline__ void pull_dir(const StepParams<T>& p, long long xc, A
     if (CY * CZ) a.pyz += T(CY * CZ) * h;
 }
 
-template <typename T, int Q, int NC>
+template <typename T, int Q, int NC, int NF = 0>
 __global__ void __launch_bounds__(256) k_step_gather(const StepParams<T> p) {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
@@ -134,7 +154,7 @@ __global__ void __launch_bounds__(256) k_step_gather(const StepParams<T> p) {
     if (x >= p.L.nx || y >= p.L.ny) return;
     const long long xc = lidx(p.L, x, y, z);
     Acc<T> a = {};
-#define LBWP_DIR(CX, CY, CZ) pull_dir<T, Q, NC, CX, CY, CZ>(p, xc, a);
+#define LBWP_DIR(CX, CY, CZ) pull_dir<T, Q, NC, CX, CY, CZ, NF>(p, xc, a);
 #define LBWP_ROW(CY, CZ) LBWP_DIR(-1, CY, CZ) LBWP_DIR(0, CY, CZ) LBWP_DIR(1, CY, CZ)
 #define LBWP_PLANE(CZ) LBWP_ROW(-1, CZ) LBWP_ROW(0, CZ) LBWP_ROW(1, CZ)
     LBWP_PLANE(-1) LBWP_PLANE(0) LBWP_PLANE(1)
@@ -189,6 +209,54 @@ __global__ void __launch_bounds__(256) k_colour_gradient(const StepParams<T> p, 
     store_images(dst3, p.L, x, y, z, gx);
     store_images(dst3 + F, p.L, x, y, z, gy);
     store_images(dst3 + 2 * F, p.L, x, y, z, gz);
+}
+
+// Near-contact repulsion F_rep = -A_h[h(x)] n delta_I (Eq. 10; readings C20-C23): at interface nodes
+// (|G| > G_I = 0.05) walk along the lattice direction closest to the outward normal -G/|G| (first in the order cz, cy,
+// cx on a tie); the first interface node within h_c whose gradient opposes G is a facing interface: F = (A_h/2) G.
+// grad3: Gx, Gy, Gz (ghost-padded); dst3: Fx, Fy, Fz with ghost images.
+template <typename T, int Q>
+__global__ void __launch_bounds__(256) k_near_contact(const StepParams<T> p, const T* __restrict__ grad3, T* __restrict__ dst3) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    const Layout& L = p.L;
+    if (x >= L.nx || y >= L.ny) return;
+    const long long xc = lidx(L, x, y, z);
+    const long long F = L.field;
+    const T gx = grad3[xc], gy = grad3[F + xc], gz = grad3[2 * F + xc];
+    T fx = T(0), fy = T(0), fz = T(0);
+    const T GI2 = T(0.05 * 0.05);
+    if (gx * gx + gy * gy + gz * gz > GI2) {
+        int mx = 0, my = 0, mz = 0;
+        T best = T(-1e30), len = T(1);
+#pragma unroll
+        for (int cz = -1; cz <= 1; ++cz)
+#pragma unroll
+            for (int cy = -1; cy <= 1; ++cy)
+#pragma unroll
+                for (int cx = -1; cx <= 1; ++cx) {
+                    const int n2 = cx * cx + cy * cy + cz * cz;
+                    if (n2 == 0 || (Q == 19 && n2 == 3)) continue;
+                    const T norm = n2 == 1 ? T(1) : n2 == 2 ? T(1.4142135623730951) : T(1.7320508075688772);
+                    const T cosv = -(T(cx) * gx + T(cy) * gy + T(cz) * gz) / norm;
+                    if (cosv > best) { best = cosv; mx = cx; my = cy; mz = cz; len = norm; }
+                }
+        for (int k = 1; T(k) * len <= p.h_c; ++k) {
+            int px = (x + k * mx) % L.nx, py = (y + k * my) % L.ny, pz = (z + k * mz) % L.nz;   // periodic (reading C13)
+            px += px < 0 ? L.nx : 0; py += py < 0 ? L.ny : 0; pz += pz < 0 ? L.nz : 0;
+            const long long pc = lidx(L, px, py, pz);
+            const T qx = grad3[pc], qy = grad3[F + pc], qz = grad3[2 * F + pc];
+            if (qx * qx + qy * qy + qz * qz > GI2 && qx * gx + qy * gy + qz * gz < T(0)) {
+                const T h = T(0.5) * p.A_h;
+                fx = h * gx; fy = h * gy; fz = h * gz;
+                break;
+            }
+        }
+    }
+    store_images(dst3, L, x, y, z, fx);
+    store_images(dst3 + F, L, x, y, z, fy);
+    store_images(dst3 + 2 * F, L, x, y, z, fz);
 }
 
 }  // namespace lbwp

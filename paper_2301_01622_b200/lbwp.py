@@ -35,7 +35,8 @@ class Params(ctypes.Structure):
                 ("ncomp", ctypes.c_int32), ("scheme", ctypes.c_int32), ("kernel", ctypes.c_int32),
                 ("nx", ctypes.c_int32), ("ny", ctypes.c_int32), ("nz", ctypes.c_int32),
                 ("device", ctypes.c_int32), ("tau", ctypes.c_double), ("A", ctypes.c_double),
-                ("beta", ctypes.c_double), ("stream", ctypes.c_void_p), ("buf", ctypes.c_void_p * 2)]
+                ("beta", ctypes.c_double), ("stream", ctypes.c_void_p), ("buf", ctypes.c_void_p * 2),
+                ("A_h", ctypes.c_double), ("h_c", ctypes.c_double)]
 
 
 class Diag(ctypes.Structure):
@@ -83,7 +84,7 @@ def _check(rc):
 
 
 def make_params(*, lattice, dtype, ncomp, shape, tau, A=0.0, beta=0.0, scheme="moments", kernel="auto",
-                device=0, stream=0, buf=(None, None)) -> Params:
+                device=0, stream=0, buf=(None, None), A_h=0.0, h_c=4.0) -> Params:
     """shape = (nz, ny, nx) as in the external layout [M, nz, ny, nx]."""
     nz, ny, nx = shape
     p = Params()
@@ -95,6 +96,7 @@ def make_params(*, lattice, dtype, ncomp, shape, tau, A=0.0, beta=0.0, scheme="m
     p.nx, p.ny, p.nz = int(nx), int(ny), int(nz)
     p.device = int(device)
     p.tau, p.A, p.beta = float(tau), float(A), float(beta)
+    p.A_h, p.h_c = float(A_h), float(h_c)
     p.stream = stream or None
     p.buf[0], p.buf[1] = buf
     return p
@@ -109,7 +111,7 @@ class Lbwp:
     CUDA tensor, external layout [M, nz, ny, nx] in the run's dtype."""
 
     def __init__(self, moments0, *, lattice=27, dtype="f32", ncomp=1, tau, A=0.0, beta=0.0,
-                 scheme="moments", kernel="auto", device=0, use_torch_buffers=True):
+                 scheme="moments", kernel="auto", device=0, use_torch_buffers=True, A_h=0.0, h_c=4.0):
         import torch  # device memory + stream only
 
         if not torch.cuda.is_available():
@@ -125,7 +127,7 @@ class Lbwp:
         self.device = torch.device("cuda", device)
         stream = torch.cuda.current_stream(self.device).cuda_stream
         p = make_params(lattice=lattice, dtype=dtype, ncomp=ncomp, shape=self.shape, tau=tau, A=A,
-                        beta=beta, scheme=scheme, kernel=kernel, device=device, stream=stream)
+                        beta=beta, scheme=scheme, kernel=kernel, device=device, stream=stream, A_h=A_h, h_c=h_c)
         self.state_bytes = state_bytes(p)
         if self.state_bytes == 0:
             raise LbwpError(-1, "invalid parameters")

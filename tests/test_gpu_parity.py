@@ -323,3 +323,29 @@ def test_diagnostics_errors(lbwp):
         assert d["count_above"] == 32 ** 3 and abs(d["rho_mean_above"] - 1.0) < 1e-15 and d["mass"][1] == 0.0
         with pytest.raises(lbwp.LbwpError):
             sim.diagnostics(0.5, [(32, 0, 0)])
+
+
+# ---- near-contact repulsion (Eq. 10; readings C20-C24): two drops pressed against
+#      each other with the force on, against the oracle; the force must act (the run differs from A_h = 0) and the
+#      momentum it injects is antisymmetric between the drops ------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("lattice", [19, 27])
+def test_near_contact_force(lbwp, oracle, dtype, lattice):
+    n, R, gap = 40, 9.0, 2.0
+    d = 2 * R + gap
+    m = wl.droplets(n, [(n / 2 - d / 2, n / 2, n / 2 - 2), (n / 2 + d / 2, n / 2, n / 2 + 2)], R, [0.03, -0.03], shape=(n, 36, 33))
+    m0 = wl.as_dtype(m, dtype)
+    kw = dict(lattice=lattice, tau=0.8, A=0.01, beta=0.7)
+    steps = 25
+    with lbwp.Lbwp(m0, dtype=dtype, ncomp=2, A_h=0.02, h_c=4.0, **kw) as sim:
+        assert sim.kernel_name == "gather%d_%s_c2" % (lattice, dtype) and sim.launches_per_step == 3
+        sim.step(steps)
+        got = sim.moments_host()
+    ref = oracle.run_nc(m0, nsteps=steps, A_h=0.02, h_c=4.0, **kw)
+    errs, _ = report("near_contact_q%d/%s/%d steps" % (lattice, dtype, steps), got, ref, 2, dtype)
+    assert errs.max() <= TOL[dtype], errs
+    assert sign_agreement(got, ref) >= 0.9999
+    off = oracle.run(m0, ncomp=2, nsteps=steps, **kw)
+    assert np.abs(ref - off).max() > 1e-3                    # the repulsion changed the collision
+    with pytest.raises(lbwp.LbwpError):                      # not built into the TMA kernels
+        lbwp.Lbwp(wl.as_dtype(wl.config3(64)["moments"], dtype), dtype=dtype, ncomp=2, A_h=0.02, kernel="tma", **kw)
