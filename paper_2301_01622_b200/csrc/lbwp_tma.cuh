@@ -159,6 +159,21 @@ __device__ __forceinline__ void consumer_release(uint32_t empty_bar, int tid) {
     __syncwarp();
     if ((tid & 31) == 0) mbar_arrive(empty_bar);
 }
+// The same guarantee without a fence (which also waits for the warp's outstanding global stores): the arrive's
+// ADDRESS is made to depend on a value `v` computed from every load of the stage (accumulators the whole plane
+// feeds), so it cannot issue before those loads have returned.  An LDS completes for the whole warp at once, so
+// lane 0's dependency covers all lanes.  `mask` is a kernel parameter that is 0 at run time: neither the compiler
+// nor ptxas can fold `bits(v) & mask` away.
+__device__ __forceinline__ void consumer_release_after(uint32_t empty_bar, int tid, float v, uint32_t mask) {
+    const uint32_t zero = __float_as_uint(v) & mask;
+    __syncwarp();
+    if ((tid & 31) == 0) mbar_arrive(empty_bar + zero);
+}
+__device__ __forceinline__ void consumer_release_after(uint32_t empty_bar, int tid, double v, uint32_t mask) {
+    const uint32_t zero = (uint32_t)__double2hiint(v) & mask;
+    __syncwarp();
+    if ((tid & 31) == 0) mbar_arrive(empty_bar + zero);
+}
 // 4-D tiled load: coordinates (x, field, y, z) of the box origin
 __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2, int c3) {
     asm volatile(

@@ -57,6 +57,7 @@ struct Tma2gParams {
     T omega, A, beta;
     int lz;
     int sh;                // x-paired mode: 1 if the CTA owns x0+1 .. x0+TX (reading buffer 0), else 0 (TmaCfg)
+    uint32_t dep_mask = 0; // always 0: makes the consumers' release data-dependent (consumer_release_after)
 };
 
 // finished sums (drho, j, dP_aa, P_ab, rhoA) of one node -> the eleven state fields (BGK in moment space, Eq. 8), with
@@ -356,7 +357,7 @@ k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant_
             for (int j = 0; j < 3; ++j) rs[n][j] = r[n][j] + s * G::STAGE;
         if constexpr (Q == 27) S::consume2c(sm, rs, P, Cc, N);
         else S::consume2c19(sm, rs, P, Cc, N);
-        consumer_release(empty(s), tid);
+        consumer_release_after(empty(s), tid, ((P[0] + Cc[0]) + (P[C::NA - 1] + Cc[C::NA - 1])).get(0), p.dep_mask);   // see lbwp_tma_kernel.cuh
         // ---- phase E: this input plane completes output plane z0 + i - 2 ----
         if (i >= 2) {
             if constexpr (C::PX != 0 && EPI == EPI_SFORM) {

@@ -260,7 +260,9 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
         else if constexpr (C::NC == 2) S::consume2c19(sm, rs, P, Cc, N);
         else if constexpr (C::Q == 27) S::consume(sm, rs, P, Cc, N);
         else S::consume19(sm, rs, P, Cc, N);
-        consumer_release(empty(s), tid);
+        // P[0] (all W and O brackets), Cc[0] (all E brackets, the D3Q19 corners included) and, for two components, the
+        // colour sums P[10], Cc[10] (rA, K, R0) together depend on every load of the plane
+        consumer_release_after(empty(s), tid, ((P[0] + Cc[0]) + (P[C::NA - 1] + Cc[C::NA - 1])).get(0), p.dep_mask);
         if (i >= 2) {                               // this input plane completes output plane z0 + i - 2
             // collision over the thread's nodes at once, except where it costs registers the stencil needs
             // (fp32 D3Q27 at 96 registers: packed epilogue spills and measured 56 vs 62 GLUPS)

@@ -14,6 +14,7 @@ struct TmaStepParams {
     int lz;                // z planes per chunk
     T beta = T(0);         // recolouring strength (fused two-component mode only)
     int sh = 0;            // x-paired mode: 1 if the CTA owns x0+1 .. x0+TX (source buffer of even parity), else 0
+    uint32_t dep_mask = 0; // always 0: makes the consumers' release data-dependent (consumer_release_after)
 };
 
 // Compile-time geometry of one instance.
