@@ -178,16 +178,13 @@ __device__ __forceinline__ void colour_unit(T* __restrict__ st, const T* __restr
         gx = w * dsum; gy = w * ysum; gz = w * zsum;
     }
     const GV g2 = vfma(gx, gx, vfma(gy, gy, gz * gz));
-    GV ig;
-#pragma unroll
-    for (int n = 0; n < GN; ++n) ig.set(n, g2.get(n) > T(1e-10) ? rsqrt_t<T>(g2.get(n)) : T(0));   // reading C8
-    const GV g = g2 * ig, nx = gx * ig, ny = gy * ig, nz = gz * ig;
     T* __restrict__ q = st + row * G::ROWP + sc;
-    // Away from the interface (n = 0 for every node of the warp's units, reading C8) both colour operators vanish
-    // identically: the S-form stays as it is and K = R0 = 0.  Exact, warp-uniform, and the common case.
+    // Away from the interface (|G|^2 <= 1e-10, i.e. n = 0, for every node of the warp's units, reading C8) both colour
+    // operators vanish identically: the S-form stays as it is and K = R0 = 0.  Exact, warp-uniform, the common case;
+    // decided before the square root is taken.
     bool flat = true;
 #pragma unroll
-    for (int n = 0; n < GN; ++n) flat = flat && ig.get(n) == T(0);
+    for (int n = 0; n < GN; ++n) flat = flat && !(g2.get(n) > T(1e-10));
     auto ldv = [&](int f) { GV v;
         if constexpr (GN == 2 && C::PX != 0) { const float2 w = *reinterpret_cast<const float2*>(q + f * C::BW); v.x = w.x; v.y = w.y; }
         else {
@@ -206,6 +203,10 @@ __device__ __forceinline__ void colour_unit(T* __restrict__ st, const T* __restr
         for (int f = 11; f < 15; ++f) stv(f, GV::bc(T(0)));
         return;
     }
+    GV ig;
+#pragma unroll
+    for (int n = 0; n < GN; ++n) ig.set(n, g2.get(n) > T(1e-10) ? rsqrt_t<T>(g2.get(n)) : T(0));   // reading C8
+    const GV g = g2 * ig, nx = gx * ig, ny = gy * ig, nz = gz * ig;
     const T cw = Q == 27 ? T(1.0 / 216.0) : T(1.0 / 36.0);
     const GV sa = ldv(0), sxx = ldv(4), syy = ldv(5), szz = ldv(6), rA = ldv(10);
     const GV rho = vfma(GV::bc(T(1) / cw), vfma(GV::bc(T(1.0 / 3.0)), sxx + syy + szz, sa), GV::bc(T(1)));
@@ -308,6 +309,10 @@ k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant_
         const int gt = tid - C::NT;
         constexpr int NU = (C::TX + 2) / GN, NUNITS = NU * G::SLOTS;
         static_assert((C::TX + 2) % GN == 0, "units tile the source row");
+        // the units this thread handles in every plane: u = gt, gt + 128, ...; (row slot, unit in row) advance by
+        // (128 / NU, 128 % NU) with a carry, no division in the plane loop
+        const int row0 = gt / NU, cu0 = gt - row0 * NU;
+        constexpr int DROW = TMA2G_G_THREADS / NU, DCU = TMA2G_G_THREADS % NU;
         int s = 0;
         uint32_t par = 0;
         for (int i = 0; i < t.nin; ++i) {
@@ -316,10 +321,12 @@ k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant_
             const T* const rm = ring + ((i + 0) % G::RNS) * G::RPLANE;   // plane z - 1 (relative index i - 1)
             const T* const rc = ring + ((i + 1) % G::RNS) * G::RPLANE;   // plane z
             const T* const rp = ring + ((i + 2) % G::RNS) * G::RPLANE;   // plane z + 1
+            int row = row0, cu = cu0;
 #pragma unroll 1
             for (int u = gt; u < NUNITS; u += TMA2G_G_THREADS) {
-                const int row = u / NU;
-                colour_unit<T, C, G, GN>(st, rm, rc, rp, row, (u - row * NU) * GN, p.A, p.beta);
+                colour_unit<T, C, G, GN>(st, rm, rc, rp, row, cu * GN, p.A, p.beta);
+                row += DROW; cu += DCU;
+                if (cu >= NU) { cu -= NU; ++row; }
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // these writes precede the stage's next TMA fill
             consumer_release(gdone(s), tid);
@@ -428,7 +435,7 @@ __global__ void __launch_bounds__(256) k_tma2g_export_raw(XLayout L, const T* __
 
 // ---- host side ---------------------------------------------------------------------------------------
 template <typename T, int Q> struct Tma2gGeom;
-template <int Q> struct Tma2gGeom<float, Q> { using C = TmaCfg<float, 2, 64, 8, 4, Q, 2, Q == 19 ? 1 : 0>; };
+template <int Q> struct Tma2gGeom<float, Q> { using C = TmaCfg<float, 2, 64, 8, 4, Q, 2, 1>; };   // x-paired consumers
 template <int Q> struct Tma2gGeom<double, Q> { using C = TmaCfg<double, 1, 32, 8, 4, Q, 2>; };
 
 struct Tma2gPlanBase {
