@@ -135,6 +135,37 @@ typedef struct lbwp_diag {
 int lbwp_diagnostics(lbwp_ctx *ctx, double threshold, int nprobes, const int32_t *probe_xyz, lbwp_diag *out,
                      double *probe_rho);
 
+/* The same reduction for callers that may not allocate: code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc.  This entry point calls no cudaMalloc / cudaFree / allocating
+ * library routine, needs no context, enqueues two kernels on `stream` and returns without synchronising.  Its only
+ * scratch (the 592 block partials of 9 doubles: LBWP_DIAG_STATIC_SCRATCH_BYTES) is a file-scope device array of the
+ * library, held by every GPU that loads the library until the process exits.
+ *   device     CUDA device ordinal in [0, LBWP_DIAG_STATIC_MAX_DEVICES) that holds every pointer below
+ *   dtype, ncomp, nx, ny, nz   as in lbwp_params; nx*ny*nz <= LBWP_DIAG_STATIC_MAX_NODES
+ *   moments    DEVICE pointer, the dense external layout of lbwp_moments: [M][nz][ny][nx], M = lbwp_num_moments(ncomp)
+ *   probe_xyz  DEVICE pointer, nprobes <= LBWP_DIAG_STATIC_MAX_PROBES triples (x, y, z); may be NULL if nprobes == 0
+ *   out        DEVICE pointer, LBWP_DIAG_STATIC_NOUT + nprobes doubles, all written by the call:
+ *              [0] sum rhoA  [1] sum rhoB  [2..4] sum rho u  [5] sum of the density over the nodes above the threshold
+ *              [6] number of those nodes  [7] 0  [8] maximum density  [9 + p] density at probe p (NaN if the probe
+ *              lies outside the box: the coordinates are device data the host cannot check)
+ *   stream     cudaStream_t (NULL: the default stream)
+ * Sums are added in the same order as lbwp_diagnostics adds them, so [0..8] equal its results bit for bit
+ * (rho_mean_above = out[5] / out[6]).
+ * The scratch is SHARED by every call on a device and keeps the last call's contents.  Nothing in it has to start at
+ * zero (the first kernel writes every element the second reads), but two calls that overlap on the GPU (different
+ * streams without an ordering between them, or concurrent branches of one graph) race on it: order them.
+ * The first call on each device resolves the array's device address (cudaGetSymbolAddress, which may load the
+ * library's module): make one call per device before starting a stream capture.
+ * LBWP_EINVAL for a NULL pointer, a bad dtype / ncomp / device, or a size beyond the maxima above (the text from
+ * lbwp_last_error names the limit); LBWP_ECUDA if the address lookup or a launch fails. */
+#define LBWP_DIAG_STATIC_SCRATCH_BYTES 42624 /* 592 blocks x 9 doubles */
+#define LBWP_DIAG_STATIC_MAX_NODES 2147483648LL /* 2^31, the library's own grid limit */
+#define LBWP_DIAG_STATIC_MAX_PROBES 4096
+#define LBWP_DIAG_STATIC_MAX_DEVICES 64
+#define LBWP_DIAG_STATIC_NOUT 9
+int lbwp_diagnostics_static(int device, int dtype, int ncomp, int nx, int ny, int nz, const void *moments,
+                            double threshold, int nprobes, const int32_t *probe_xyz, double *out, void *stream);
+
 /* z-slab decomposition over several GPUs (the paper's motivation are grids of billions of nodes,
  * PAPER.md:163-167).  A rank's context is an ordinary periodic box whose first and last H planes are HALO planes:
  * copies of the neighbouring ranks' boundary planes (H = 1; H = 2 for ncomp == 2 moments, whose colour gradient

@@ -6,6 +6,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "../../include/lbwp.h"
@@ -575,6 +576,69 @@ int lbwp_diagnostics(lbwp_ctx* c, double threshold, int nprobes, const int32_t* 
     out->rho_mean_above = h[6] > 0.0 ? h[5] / h[6] : 0.0;
     out->rho_max = h[lbwp::DIAG_NSUM];
     for (int p = 0; p < nprobes; ++p) probe_rho[p] = h[NP + p];
+    return LBWP_OK;
+}
+
+// ---- lbwp_diagnostics_static: the same reduction with no allocation anywhere (include/lbwp.h) ----------------------
+// The block partials live in this file-scope device array.  In host code its name is a host-side stand-in, not a device
+// address: the address a kernel may use is looked up once per device (that device current) and cached.
+static __device__ __align__(256) double g_diag_static_scratch[lbwp::DIAG_BLOCKS * (lbwp::DIAG_NSUM + 1)];
+static_assert(sizeof(g_diag_static_scratch) == LBWP_DIAG_STATIC_SCRATCH_BYTES, "include/lbwp.h states the scratch size");
+static_assert(LBWP_DIAG_STATIC_NOUT == lbwp::DIAG_NSUM + 1, "include/lbwp.h states the output layout");
+
+namespace {
+std::mutex g_diag_static_mu;
+double* g_diag_static_addr[LBWP_DIAG_STATIC_MAX_DEVICES] = {};
+
+// `device` is current.  cudaGetSymbolAddress resolves the array in the current device's copy of the module.
+int diag_static_scratch(int device, double** ptr) {
+    std::lock_guard<std::mutex> lock(g_diag_static_mu);
+    if (!g_diag_static_addr[device]) {
+        void* p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_diag_static_scratch));
+        if (!p) return fail(LBWP_ECUDA, "lbwp_diagnostics_static: cudaGetSymbolAddress returned NULL on device %d", device);
+        g_diag_static_addr[device] = (double*)p;
+    }
+    *ptr = g_diag_static_addr[device];
+    return LBWP_OK;
+}
+}  // namespace
+
+int lbwp_diagnostics_static(int device, int dtype, int ncomp, int nx, int ny, int nz, const void* moments, double threshold,
+                            int nprobes, const int32_t* probe_xyz, double* out, void* stream) {
+    if (!moments || !out) return fail(LBWP_EINVAL, "lbwp_diagnostics_static: moments or out is NULL");
+    if (dtype != LBWP_F32 && dtype != LBWP_F64) return fail(LBWP_EINVAL, "lbwp_diagnostics_static: dtype %d is neither LBWP_F32 nor LBWP_F64", dtype);
+    if (ncomp != 1 && ncomp != 2) return fail(LBWP_EINVAL, "lbwp_diagnostics_static: ncomp %d is neither 1 nor 2", ncomp);
+    if (device < 0 || device >= LBWP_DIAG_STATIC_MAX_DEVICES)
+        return fail(LBWP_EINVAL, "lbwp_diagnostics_static: device %d outside [0, %d)", device, LBWP_DIAG_STATIC_MAX_DEVICES);
+    if (nx < 1 || ny < 1 || nz < 1) return fail(LBWP_EINVAL, "lbwp_diagnostics_static: empty box %d x %d x %d", nx, ny, nz);
+    if ((double)nx * (double)ny * (double)nz > (double)LBWP_DIAG_STATIC_MAX_NODES)
+        return fail(LBWP_EINVAL, "lbwp_diagnostics_static: %d x %d x %d nodes exceed the maximum of %lld (LBWP_DIAG_STATIC_MAX_NODES)",
+                    nx, ny, nz, (long long)LBWP_DIAG_STATIC_MAX_NODES);
+    if (nprobes < 0 || nprobes > LBWP_DIAG_STATIC_MAX_PROBES)
+        return fail(LBWP_EINVAL, "lbwp_diagnostics_static: %d probes outside [0, %d] (LBWP_DIAG_STATIC_MAX_PROBES)", nprobes,
+                    LBWP_DIAG_STATIC_MAX_PROBES);
+    if (nprobes > 0 && !probe_xyz) return fail(LBWP_EINVAL, "lbwp_diagnostics_static: probe_xyz is NULL with %d probes", nprobes);
+    DeviceGuard guard(device);
+    if (!guard.ok) return fail(LBWP_ECUDA, "cudaSetDevice(%d) failed", device);
+    double* partial = nullptr;
+    int rc = diag_static_scratch(device, &partial);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long n = (long long)nx * ny * nz;
+    const int* probes = (const int*)probe_xyz;
+    if (dtype == LBWP_F32) {
+        const float* m = (const float*)moments;
+        if (ncomp == 1) lbwp::k_diag_partial<float, 1><<<lbwp::DIAG_BLOCKS, lbwp::DIAG_THREADS, 0, st>>>(m, n, threshold, partial);
+        else lbwp::k_diag_partial<float, 2><<<lbwp::DIAG_BLOCKS, lbwp::DIAG_THREADS, 0, st>>>(m, n, threshold, partial);
+        lbwp::k_diag_final_checked<float><<<1, 128, 0, st>>>(partial, lbwp::DIAG_BLOCKS, m, nx, ny, nz, probes, nprobes, out);
+    } else {
+        const double* m = (const double*)moments;
+        if (ncomp == 1) lbwp::k_diag_partial<double, 1><<<lbwp::DIAG_BLOCKS, lbwp::DIAG_THREADS, 0, st>>>(m, n, threshold, partial);
+        else lbwp::k_diag_partial<double, 2><<<lbwp::DIAG_BLOCKS, lbwp::DIAG_THREADS, 0, st>>>(m, n, threshold, partial);
+        lbwp::k_diag_final_checked<double><<<1, 128, 0, st>>>(partial, lbwp::DIAG_BLOCKS, m, nx, ny, nz, probes, nprobes, out);
+    }
+    CU(cudaGetLastError());
     return LBWP_OK;
 }
 

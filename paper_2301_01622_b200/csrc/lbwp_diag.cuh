@@ -75,4 +75,25 @@ __global__ void k_diag_final(const double* __restrict__ partial, int blocks, con
     }
 }
 
+// k_diag_final for probe coordinates the host never saw (lbwp_diagnostics_static: they are device data): the same sums
+// in the same order; a probe outside the box reads nothing and reports NaN; out[DIAG_NSUM - 1] (unused sum) is 0.
+template <typename T>
+__global__ void k_diag_final_checked(const double* __restrict__ partial, int blocks, const T* __restrict__ m, int nx, int ny, int nz,
+                                     const int* __restrict__ probes, int nprobes, double* __restrict__ out /* [NSUM + 1 + nprobes] */) {
+    const int k = threadIdx.x;
+    if (k <= DIAG_NSUM) {
+        double a = partial[k];
+        for (int b = 1; b < blocks; ++b) {
+            const double v = partial[(long long)b * (DIAG_NSUM + 1) + k];
+            a = k == DIAG_NSUM ? (v > a ? v : a) : a + v;
+        }
+        out[k] = a;
+    }
+    for (int p = k; p < nprobes; p += blockDim.x) {
+        const int x = probes[3 * p], y = probes[3 * p + 1], z = probes[3 * p + 2];
+        const bool inside = x >= 0 && x < nx && y >= 0 && y < ny && z >= 0 && z < nz;
+        out[DIAG_NSUM + 1 + p] = inside ? (double)m[((long long)z * ny + y) * nx + x] : __longlong_as_double(0x7ff8000000000000ll);
+    }
+}
+
 }  // namespace lbwp

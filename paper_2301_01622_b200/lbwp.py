@@ -20,6 +20,7 @@ LBWP_F32, LBWP_F64 = 0, 1
 LBWP_MOMENTS, LBWP_POPULATIONS = 0, 1
 KERNELS = {"auto": 0, "gather": 1, "march": 2, "tma": 3, "tma_split": 4}
 EXPORTS = ["lbwp_state_bytes", "lbwp_num_moments", "lbwp_init", "lbwp_step", "lbwp_moments", "lbwp_diagnostics",
+           "lbwp_diagnostics_static",
            "lbwp_halo_bytes", "lbwp_halo_pack", "lbwp_halo_unpack", "lbwp_set_moments", "lbwp_steps_done", "lbwp_launches_per_step", "lbwp_kernel_name",
            "lbwp_sync", "lbwp_destroy", "lbwp_last_error"]
 
@@ -65,6 +66,8 @@ def load():
     lib.lbwp_set_moments.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]
     lib.lbwp_diagnostics.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_int, ctypes.POINTER(ctypes.c_int32),
                                      ctypes.POINTER(Diag), ctypes.POINTER(ctypes.c_double)]
+    lib.lbwp_diagnostics_static.argtypes = [ctypes.c_int] * 6 + [ctypes.c_void_p, ctypes.c_double, ctypes.c_int,
+                                            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
     lib.lbwp_halo_bytes.argtypes, lib.lbwp_halo_bytes.restype = [ctypes.c_void_p, ctypes.c_int], ctypes.c_size_t
     lib.lbwp_halo_pack.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p]
     lib.lbwp_halo_unpack.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p]
@@ -104,6 +107,40 @@ def make_params(*, lattice, dtype, ncomp, shape, tau, A=0.0, beta=0.0, scheme="m
 
 def state_bytes(params: Params) -> int:
     return int(load().lbwp_state_bytes(ctypes.byref(params)))
+
+
+# limits of lbwp_diagnostics_static as include/lbwp.h states them
+DIAG_STATIC_SCRATCH_BYTES = 42624
+DIAG_STATIC_MAX_NODES = 1 << 31
+DIAG_STATIC_MAX_PROBES = 4096
+DIAG_STATIC_NOUT = 9
+
+
+def diagnostics_static(moments, out, *, ncomp, threshold=0.5, probes=None, shape=None):
+    """lbwp_diagnostics_static: the diagnostics of dense moments the CALLER holds, with no allocation in the library
+    (its scratch is a static device array; calls that overlap on the GPU race on it).  Asynchronous on torch's current
+    stream of the tensors' device.
+
+    moments: contiguous CUDA tensor [M, nz, ny, nx], float32 or float64 (`shape` = (nz, ny, nx) overrides the tensor's
+    own box, for callers that view a larger buffer); probes: None or a contiguous int32 CUDA tensor [n, 3] of
+    (x, y, z); out: contiguous float64 CUDA tensor of at least 9 + n elements, written as include/lbwp.h lists."""
+    import torch  # device pointers and the current stream only
+
+    if not (moments.is_cuda and moments.is_contiguous() and moments.dtype in (torch.float32, torch.float64)):
+        raise ValueError("moments must be a contiguous float32/float64 CUDA tensor")
+    nz, ny, nx = (int(v) for v in (shape if shape is not None else moments.shape[1:]))
+    n = 0 if probes is None else int(probes.shape[0])
+    if n and not (probes.is_cuda and probes.is_contiguous() and probes.dtype == torch.int32 and probes.device == moments.device
+                  and probes.dim() == 2 and probes.shape[1] == 3):
+        raise ValueError("probes must be a contiguous int32 CUDA tensor [n, 3] on the moments' device")
+    if not (out.is_cuda and out.is_contiguous() and out.dtype == torch.float64 and out.device == moments.device
+            and out.numel() >= DIAG_STATIC_NOUT + n):
+        raise ValueError("out must be a contiguous float64 CUDA tensor of at least 9 + nprobes elements on the moments' device")
+    dev = moments.device.index if moments.device.index is not None else torch.cuda.current_device()
+    _check(load().lbwp_diagnostics_static(dev, LBWP_F32 if moments.dtype == torch.float32 else LBWP_F64, int(ncomp), nx, ny, nz,
+                                          ctypes.c_void_p(moments.data_ptr()), float(threshold), n,
+                                          ctypes.c_void_p(probes.data_ptr()) if n else None, ctypes.c_void_p(out.data_ptr()),
+                                          ctypes.c_void_p(torch.cuda.current_stream(moments.device).cuda_stream)))
 
 
 class Lbwp:
