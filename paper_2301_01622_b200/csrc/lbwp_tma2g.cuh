@@ -278,13 +278,14 @@ k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant_
         auto wrapy = [&](int y) { return y < 0 ? y + L.ny : (y >= L.ny ? y - L.ny : y); };
         const int bx = C::PX ? t.x0 + 16 / (int)sizeof(T) : t.x0 + L.ox - C::OX;   // stage box start column (16-byte aligned)
         const int rbx = bx - G::RCO;
+        const uint64_t keep = l2_policy_evict_last();
         // rA plane of relative index i (plane z0 - 1 + i) -> ring slot (i + 1) % RNS
         auto load_ra = [&](int i, uint32_t bar) {
             const int z = wrapz(wrapz(t.z0 - 1 + i));
             const uint32_t dst = ring_u32 + (uint32_t)(((i + 1) % G::RNS) * G::RPLANE * sizeof(T));
-            tma_load_4d(dst, &map_ra2, bar, rbx, 10, wrapy(t.y0 - 2), z);
-            tma_load_4d(dst + (uint32_t)(2 * G::RBW * sizeof(T)), &map_ra8, bar, rbx, 10, t.y0, z);
-            tma_load_4d(dst + (uint32_t)((2 + C::TY) * G::RBW * sizeof(T)), &map_ra2, bar, rbx, 10, wrapy(t.y0 + C::TY), z);
+            tma_load_4d(dst, &map_ra2, bar, rbx, 10, wrapy(t.y0 - 2), z, keep);
+            tma_load_4d(dst + (uint32_t)(2 * G::RBW * sizeof(T)), &map_ra8, bar, rbx, 10, t.y0, z, keep);
+            tma_load_4d(dst + (uint32_t)((2 + C::TY) * G::RBW * sizeof(T)), &map_ra2, bar, rbx, 10, wrapy(t.y0 + C::TY), z, keep);
         };
         int ps = 0;
         uint32_t pround = 0;
@@ -297,7 +298,7 @@ k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant_
             load_ra(i + 1, full(ps));
 #pragma unroll 1
             for (int r = 0; r < G::SLOTS; ++r)
-                tma_load_4d(dst + (uint32_t)(r * G::ROWP * sizeof(T)), &map_row, full(ps), bx, 0, wrapy(t.y0 - 1 + r), z);
+                tma_load_4d(dst + (uint32_t)(r * G::ROWP * sizeof(T)), &map_row, full(ps), bx, 0, wrapy(t.y0 - 1 + r), z, keep);
             if (++ps == G::NS) { ps = 0; ++pround; }
         }
         return;

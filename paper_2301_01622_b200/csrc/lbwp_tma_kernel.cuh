@@ -200,6 +200,7 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
         // ---- producer warpgroup: one lane fills every free stage, up to NS planes ahead of the consumers ----
         setmaxnreg_dec<TMA_PRODUCER_REGS>();
         if (tid != C::NT) return;
+        const uint64_t keep = l2_policy_evict_last();
         int ps = 0;
         uint32_t pround = 0;
         for (; item < nitems; item += gridDim.x) {
@@ -211,9 +212,9 @@ k_step_tma27(const __grid_constant__ CUtensorMap map_main, const __grid_constant
                 const uint32_t dst = base + (uint32_t)(ps * C::STAGE * sizeof(T));
                 mbar_expect_tx(full(ps), C::STAGE_TX_BYTES);
                 const int bx = C::PX ? t.x0 + 16 / (int)sizeof(T) : t.x0 + L.ox - C::OX;   // box start column (16-byte aligned)
-                tma_load_4d(dst, &map_main, full(ps), bx, 0, t.y0, z);
-                tma_load_4d(dst + (uint32_t)(C::OFF_YM * sizeof(T)), &map_row, full(ps), bx, 0, t.ym, z);
-                tma_load_4d(dst + (uint32_t)(C::OFF_YP * sizeof(T)), &map_row, full(ps), bx, 0, t.yp, z);
+                tma_load_4d(dst, &map_main, full(ps), bx, 0, t.y0, z, keep);
+                tma_load_4d(dst + (uint32_t)(C::OFF_YM * sizeof(T)), &map_row, full(ps), bx, 0, t.ym, z, keep);
+                tma_load_4d(dst + (uint32_t)(C::OFF_YP * sizeof(T)), &map_row, full(ps), bx, 0, t.yp, z, keep);
                 if (++ps == C::NS) { ps = 0; ++pround; }
             }
         }
