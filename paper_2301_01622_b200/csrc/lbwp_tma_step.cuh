@@ -332,8 +332,10 @@ struct TmaStep {
         ao = vfma(four, AO[1], AO[2] + AO[0]);
     }
 
+    // kzero: the plane's K and R0 fields are identically zero (and were not written: lbwp_tma2g.cuh, plane-level
+    // shortcut); their terms are skipped, which leaves the sums bit for bit as adding the zeros would.
     __device__ static __forceinline__ void consume2c(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
-                                                     V (&Cc)[C::NA], V (&N)[C::NA]) {
+                                                     V (&Cc)[C::NA], V (&N)[C::NA], bool kzero = false) {
         const V four = V::bc(T(4));
         V El[3], Wl[3], Ol[3], Em[3], Wm[3], Om[3], Eh[3], Wh[3], Oh[3];
         brackets_any<-1, true>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
@@ -354,6 +356,12 @@ struct TmaStep {
         colour_row<1>(s, r, Eh, Wh, Oh, four, aeh, awh, aoh);
         colour_row<0>(s, r, Em, Wm, Om, four, aem, awm, aom);
         const V mae = vfma(four, aem, aeh + ael), maw = vfma(four, awm, awh + awl), mao = vfma(four, aom, aoh + aol);
+        if (kzero) {
+            Cc[10] = vfma(four, mae, Cc[10]);
+            N[10] = maw + mao;
+            P[10] = P[10] + (maw - mao);
+            return;
+        }
         // second part: sum_{c != 0} w_c K.c / |c|; weights x 216 / |c|: 16 (axis), 4/sqrt2 (face), 1/sqrt3 (corner)
         V kx0[3], kx1[3], kx2[3], ky0[3], ky2[3], kz0[3], kz1[3], kz2[3];   // K_a at row slot 0 (cy = +1), 1, 2
         ld3any<11>(s, r, 0, kx0); ld3any<11>(s, r, 1, kx1); ld3any<11>(s, r, 2, kx2);
@@ -396,7 +404,7 @@ struct TmaStep {
     }
 
     __device__ static __forceinline__ void consume2c19(const T* __restrict__ s, const int (&r)[C::NPT][3], V (&P)[C::NA],
-                                                       V (&Cc)[C::NA], V (&N)[C::NA]) {
+                                                       V (&Cc)[C::NA], V (&N)[C::NA], bool kzero = false) {
         const V two = V::bc(T(2)), eight = V::bc(T(8));
         V El[3], Wl[3], Ol[3], Em[3], Wm[3], Om[3], Eh[3], Wh[3], Oh[3];
         brackets_any<-1, false>(s, r, El, Wl, Ol);   // sources at y+1 (cy = -1)
@@ -413,6 +421,12 @@ struct TmaStep {
         const V mae = vfma(eight, AEm[1], vfma(two, rm, rh + rl));
         const V maw = vfma(two, AWm[1], (AWm[2] + AWm[0]) + (AWh[1] + AWl[1]));
         const V mao = vfma(two, AOm[1], (AOm[2] + AOm[0]) + (AOh[1] + AOl[1]));
+        if (kzero) {
+            Cc[10] = Cc[10] + mae;
+            N[10] = maw + mao;
+            P[10] = P[10] + (maw - mao);
+            return;
+        }
         // second part: sum_{c != 0} w_c K.c / |c|; weights x 36 / |c|: 2 (axis), 1/sqrt2 (face diagonal)
         V kx0[3], kx1[3], kx2[3], ky0[3], ky2[3], kz1[3];
         ld3any<11>(s, r, 0, kx0); ld3any<11>(s, r, 1, kx1); ld3any<11>(s, r, 2, kx2);
