@@ -349,7 +349,7 @@ k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant_
         static_assert(TMA2G_G_THREADS == 128, "four flag words per buffer");
         int s = 0;
         uint32_t par = 0;
-        int fm = 0, fc = 0, fp = 0;
+        int fm = 0, fc = 0, fp = 0, mixed_run = 0;
         for (int i = 0; i < t.nin; ++i) {
             mbar_wait(full(s), par);
             T* const st = sm + s * G::STAGE;
@@ -357,7 +357,13 @@ k_step_tma2g(const __grid_constant__ CUtensorMap map_row, const __grid_constant_
             const T* const rc = ring + ((i + 1) % G::RNS) * G::RPLANE;   // plane z
             const T* const rp = ring + ((i + 2) % G::RNS) * G::RPLANE;   // plane z + 1
             if (i == 0) { fc = classify(rm); fp = classify(rc); }        // the first stage brings three ring planes
-            fm = fc; fc = fp; fp = classify(rp);
+            // "mixed" is always a safe class (the per-unit path is exact), so inside an interface region -- four mixed
+            // planes in a row -- only every fourth plane is looked at until a bulk plane turns up again: the scan sits
+            // on the critical path of the plane (its class is needed the moment it arrives)
+            fm = fc; fc = fp;
+            if (mixed_run >= 4 && (i & 3) != 0) fp = 0;
+            else fp = classify(rp);
+            mixed_run = fp == 0 ? mixed_run + 1 : 0;
             // one bulk phase as far as this plane's gradients reach: the S-form stays, K = R0 = 0 are not even written
             // (the consumers are told through kflat[s] and skip those terms; published by the arrive on gdone below)
             const bool bulk = fm != 0 && fm == fc && fc == fp;
