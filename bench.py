@@ -50,6 +50,9 @@ def parse_args():
     ap.add_argument("--ncomp", type=int, default=1, choices=[1, 2])
     ap.add_argument("--scheme", default="moments", choices=["moments", "populations"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "gather", "march", "tma", "tma_split"])
+    ap.add_argument("--near-contact", type=float, default=0.0, metavar="A_h",
+                    help="two-component runs: strength of the near-contact repulsion (PAPER.md:93-112, Eq. 10; h_c = 4); "
+                         "0 = off.  The paper's own benchmark (PAPER.md:158-163) is --n 128 --lattice 19 --ncomp 2 with it on")
     ap.add_argument("--e2e-steps", type=int, default=2, help="host-buffer steps timed for the e2e key (0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sizes", action="store_true", help="skip the 256^3 / 512^3 fp32 / fp64 sub-record")
@@ -60,7 +63,8 @@ def parse_args():
 def workload_name(a):
     return (f"config5 sweep instance: D3Q{a.lattice} {'single' if a.ncomp == 1 else 'two'}-component "
             f"{a.scheme} {a.dtype} {a.n}^3 periodic, seeded as config 1 (Taylor-Green, tau="
-            f"{'0.8' if a.ncomp == 1 else '1.0'})")
+            f"{'0.8' if a.ncomp == 1 else '1.0'})"
+            + (f", near-contact force A_h={a.near_contact:g}, h_c=4" if a.ncomp == 2 and a.near_contact else ""))
 
 
 def algorithmic_bytes_per_lu(a):
@@ -261,7 +265,8 @@ def main():
         cfg = wl.sweep_case(b.n, b.lattice, b.ncomp, b.dtype)
         m0 = wl.as_dtype(cfg["moments"], b.dtype)
         return lbwp.Lbwp(m0, lattice=b.lattice, dtype=b.dtype, ncomp=b.ncomp, tau=cfg["tau"], A=cfg["A"],
-                         beta=cfg["beta"], scheme=b.scheme, kernel=b.kernel, device=local), m0
+                         beta=cfg["beta"], scheme=b.scheme, kernel=b.kernel, device=local,
+                         A_h=getattr(b, "near_contact", 0.0) if b.ncomp == 2 else 0.0), m0
 
     peak, peak_src = measured_peak()
     nodes = a.n ** 3
