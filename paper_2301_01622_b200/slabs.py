@@ -103,6 +103,9 @@ class SlabLbwp:
         self.halo = halo_width(lbwp_kwargs.get("ncomp", 1))
         if lbwp_kwargs.get("scheme", "moments") != "moments":
             raise ValueError("slab decomposition: moments scheme only")
+        if lbwp_kwargs.get("A_h", 0.0):
+            raise ValueError("slab decomposition: the near-contact force looks h_c + 1 planes beyond a node "
+                             "(interface walk plus gradient), more than the halo carries; not supported")
         self.sim = lbwp.Lbwp(local_m0, **lbwp_kwargs)
         self.nz_local = self.sim.shape[0]
         self.owned = self.nz_local - 2 * self.halo

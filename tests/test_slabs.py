@@ -41,6 +41,14 @@ def test_local_planes_wrap():
         slabs.slab_range(2, 3, 0)
 
 
+def test_slab_rejects_what_the_halo_cannot_carry():
+    m = np.zeros((11, 8, 8, 64), dtype=np.float32)
+    with pytest.raises(ValueError, match="near-contact"):
+        slabs.SlabLbwp(m, world=2, rank=0, ncomp=2, tau=1.0, A=0.01, beta=0.7, A_h=0.01)
+    with pytest.raises(ValueError, match="moments scheme"):
+        slabs.SlabLbwp(m, world=2, rank=0, ncomp=2, tau=1.0, scheme="populations")
+
+
 # ---- the exchange itself over gloo: a 3-point stencil in z on a decomposed periodic array ------------------------------
 def _stencil_worker(rank, world, port, nz, halo, steps, out):
     sys.path.insert(0, ROOT)
