@@ -55,9 +55,8 @@ enum lbwp_kernel {
     LBWP_KERNEL_TMA_SPLIT = 4, /* two-component only: collide pass + TMA stencil pass (the paper's split form),
                                kept for comparison with the fused form LBWP_KERNEL_TMA uses */
     LBWP_KERNEL_TMA = 3     /* TMA-fed stencil on the collided ("S-form") moments, collision as epilogue:
-                               D3Q27 and D3Q19, nx a multiple of 64 (fp32) / 32 (fp64), ny of 8; two-component runs
-                               take two launches per step (the stencil with the colour operators, then the
-                               phase-field gradient) */
+                               D3Q27 and D3Q19, nx a multiple of 64 (fp32) / 32 (fp64), ny of 8; one launch per step,
+                               two-component runs included (gradient, perturbation and recolouring fused in) */
 };
 
 typedef struct lbwp_params {
@@ -79,9 +78,12 @@ typedef struct lbwp_params {
     double A_h;          /* ncomp == 2, moments scheme: strength of the near-contact repulsion
                             F_rep = -A_h[h(x)] n delta_I (Eq. 10; readings C20-C24 of DESIGN.md:
                             delta_I = |grad phi|/2, n the outward normal, A_h[h] = A_h for h <= h_c and 0 beyond,
-                            Guo forcing).  0 = off (BASELINE's configs).  Non-zero selects the generic kernel
-                            (three launches per step: gradient, contact search, step); LBWP_EUNSUPPORTED with
-                            LBWP_KERNEL_TMA / TMA_SPLIT / MARCH. */
+                            Guo forcing).  0 = off (BASELINE's configs).  Non-zero adds a second launch per step behind
+                            the fused two-component TMA kernel (a pointwise pass that finds the facing interfaces
+                            and applies the forcing to the collided moments in place), or, for boxes the TMA tiles
+                            do not divide and with LBWP_KERNEL_GATHER, selects the generic kernel (three launches
+                            per step: gradient, contact search, step); LBWP_EUNSUPPORTED with LBWP_KERNEL_TMA_SPLIT /
+                            MARCH and in the lbwp_halo_* calls (the force looks h_c + 1 planes beyond a node). */
     double h_c;          /* cut-off distance of the near-contact force in lattice units (> 0 when A_h != 0) */
 } lbwp_params;
 

@@ -19,6 +19,7 @@
 #include "lbwp_tma_host.cuh"
 #include "lbwp_tma2.cuh"
 #include "lbwp_tma2g.cuh"
+#include "lbwp_contact.cuh"
 
 namespace {
 
@@ -88,8 +89,13 @@ bool tma2_fused(const lbwp_params* p) { return p->ncomp == 2 && p->kernel != LBW
 
 // kernel variant a context with these params runs (LBWP_KERNEL_AUTO resolved); 0 if not built
 int choose_variant(const lbwp_params* p) {
-    if (p->A_h != 0.0)   // near-contact force: built into the generic kernels only
-        return (p->kernel == LBWP_KERNEL_AUTO || p->kernel == LBWP_KERNEL_GATHER) ? LBWP_KERNEL_GATHER : 0;
+    if (p->A_h != 0.0) {   // near-contact force: a fix-up pass behind the fused two-component TMA step, or the generic kernels
+        if (p->kernel == LBWP_KERNEL_AUTO || p->kernel == LBWP_KERNEL_TMA) {
+            if (tma_eligible(p)) return LBWP_KERNEL_TMA;
+            return p->kernel == LBWP_KERNEL_AUTO ? LBWP_KERNEL_GATHER : 0;
+        }
+        return p->kernel == LBWP_KERNEL_GATHER ? LBWP_KERNEL_GATHER : 0;
+    }
     const bool march_ok = p->scheme == LBWP_MOMENTS && p->ncomp == 1 && p->lattice == 27;
     switch (p->kernel) {
         case LBWP_KERNEL_AUTO: return tma_eligible(p) ? LBWP_KERNEL_TMA : march_ok ? LBWP_KERNEL_MARCH : LBWP_KERNEL_GATHER;
@@ -345,19 +351,32 @@ struct Tma2gCtx final : lbwp_ctx {
         if (rc) return fail(rc < 0 ? LBWP_EUNSUPPORTED : LBWP_ECUDA, "fused two-component TMA plan setup failed (%d)", rc);
         return LBWP_OK;
     }
+    // near-contact force (lbwp_contact.cuh): Guo's forcing applied to the collided moments of buffer b, in place
+    int contact_fixup(int b) {
+        if (P.A_h == 0.0) return LBWP_OK;
+        lbwp::ContactParams<T> cp;
+        cp.L = planp->Lb[b]; cp.state = (T*)buf[b];
+        cp.omega = T(1.0 / P.tau); cp.A_h = T(P.A_h); cp.h_c = T(P.h_c);
+        const dim3 blk(32, 8, 1), g((X.nx + 31) / 32, (X.ny + 7) / 8, X.nz);
+        if (P.lattice == 27) lbwp::k_contact_fixup<T, 27><<<g, blk, 0, stream>>>(cp);
+        else lbwp::k_contact_fixup<T, 19><<<g, blk, 0, stream>>>(cp);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return fail(LBWP_ECUDA, "near-contact fix-up launch: %s", cudaGetErrorString(e));
+        return LBWP_OK;
+    }
     int step_once() override {
         int rc = planp->stencil(lbwp::EPI_SFORM, cur, buf[cur ^ 1], 1.0 / P.tau, P.A, P.beta, stream);
         if (rc) return fail(LBWP_ECUDA, "fused two-component step launch: %s", cudaGetErrorString((cudaError_t)rc));
         cur ^= 1;
         ++steps;
-        return LBWP_OK;
+        return contact_fixup(cur);
     }
     int import_dense(const void* ext) override {
         steps = 0;
         cur = 0;
         int rc = planp->import_state(ext, buf[0], buf[1], 1.0 / P.tau, stream);
         if (rc) return fail(LBWP_ECUDA, "import launch: %s", cudaGetErrorString((cudaError_t)rc));
-        return LBWP_OK;
+        return contact_fixup(0);
     }
     void plane_geometry(long long* field, long long* plane, long long* z0off, int* nf) const override {
         *field = X.field; *plane = X.plane; *z0off = 0; *nf = 11;
@@ -489,7 +508,7 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
     if (variant == LBWP_KERNEL_TMA) {
         if (tma2_fused(p)) {
             rc = p->dtype == LBWP_F32 ? static_cast<Tma2gCtx<float>*>(c)->prepare() : static_cast<Tma2gCtx<double>*>(c)->prepare();
-            c->launches_per_step = 1;
+            c->launches_per_step = p->A_h != 0.0 ? 2 : 1;   // + the near-contact fix-up pass
         } else if (p->ncomp == 2) {
             rc = p->dtype == LBWP_F32 ? static_cast<Tma2Ctx<float>*>(c)->prepare() : static_cast<Tma2Ctx<double>*>(c)->prepare();
             c->launches_per_step = 2;
@@ -646,6 +665,7 @@ namespace {
 int halo_copy(lbwp_ctx* c, int z0, int nplanes, void* packed, bool pack) {
     if (!c || !packed) return fail(LBWP_EINVAL, "lbwp_halo_*: NULL argument");
     if (c->P.scheme != LBWP_MOMENTS) return fail(LBWP_EUNSUPPORTED, "lbwp_halo_*: moments scheme only");
+    if (c->P.A_h != 0.0) return fail(LBWP_EUNSUPPORTED, "lbwp_halo_*: the near-contact force reaches h_c + 1 planes, more than the halo carries");
     if (nplanes < 1 || z0 < 0 || z0 + nplanes > c->L.nz) return fail(LBWP_EINVAL, "lbwp_halo_*: planes [%d, %d) leave the box", z0, z0 + nplanes);
     DeviceGuard guard(c->P.device);
     if (!guard.ok) return fail(LBWP_ECUDA, "cudaSetDevice(%d) failed", c->P.device);

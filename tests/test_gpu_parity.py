@@ -347,5 +347,40 @@ def test_near_contact_force(lbwp, oracle, dtype, lattice):
     assert sign_agreement(got, ref) >= 0.9999
     off = oracle.run(m0, ncomp=2, nsteps=steps, **kw)
     assert np.abs(ref - off).max() > 1e-3                    # the repulsion changed the collision
-    with pytest.raises(lbwp.LbwpError):                      # not built into the TMA kernels
-        lbwp.Lbwp(wl.as_dtype(wl.config3(64)["moments"], dtype), dtype=dtype, ncomp=2, A_h=0.02, kernel="tma", **kw)
+    with pytest.raises(lbwp.LbwpError):                      # not built into the split TMA form
+        lbwp.Lbwp(wl.as_dtype(wl.config3(64)["moments"], dtype), dtype=dtype, ncomp=2, A_h=0.02, kernel="tma_split", **kw)
+
+
+# the same force behind the fused two-component TMA kernel (a fix-up pass on the collided moments, lbwp_contact.cuh):
+# a box the tiles divide, the drops pressed against each other across tile, chunk and periodic boundaries
+@pytest.mark.parametrize("lattice", [19, 27])
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_near_contact_force_fused(lbwp, oracle, dtype, lattice):
+    shape = (64, 40, 36)
+    nx, ny, nz = shape
+    R, gap = 9.0, 2.0
+    d = 2 * R + gap
+    # the film between the drops lies on the periodic x boundary (ghost columns) and on a tile boundary in y
+    centres = [(nx - d / 2, 16.0, nz / 2 - 2), (d / 2, 16.0, nz / 2 + 2)]
+    m = wl.droplets(0, centres, R, [0.03, -0.03], shape=shape)
+    m0 = wl.as_dtype(m, dtype)
+    kw = dict(lattice=lattice, tau=0.8, A=0.01, beta=0.7)
+    steps = 25
+    with lbwp.Lbwp(m0, dtype=dtype, ncomp=2, A_h=0.02, h_c=4.0, **kw) as sim:
+        assert sim.kernel_name == "tma%d_%s_c2" % (lattice, dtype) and sim.launches_per_step == 2
+        sim.step(steps)
+        got = sim.moments_host()
+        sim.step(1)                                          # lbwp_moments after a further step: the export path
+        got1 = sim.moments_host()
+    ref = oracle.run_nc(m0, nsteps=steps, A_h=0.02, h_c=4.0, **kw)
+    errs, _ = report("near_contact_fused_q%d/%s/%d steps" % (lattice, dtype, steps), got, ref, 2, dtype)
+    assert errs.max() <= TOL[dtype], errs
+    assert sign_agreement(got, ref) >= 0.9999
+    ref1 = oracle.run_nc(ref, nsteps=1, A_h=0.02, h_c=4.0, **kw)
+    assert parity_errors(got1, ref1, 2, dtype).max() <= TOL[dtype]
+    off = oracle.run(m0, ncomp=2, nsteps=steps, **kw)
+    assert np.abs(ref - off).max() > 1e-3                    # the repulsion changed the collision
+    with lbwp.Lbwp(m0, dtype=dtype, ncomp=2, A_h=0.02, h_c=4.0, kernel="gather", **kw) as sim:   # and the generic path agrees
+        sim.step(steps)
+        gen = sim.moments_host()
+    assert parity_errors(got, gen.astype(np.float64), 2, dtype).max() <= TOL[dtype]
