@@ -3,6 +3,7 @@
 // ("Flip-Flop") and kernel selection.  No CPU fallback exists.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -341,6 +342,7 @@ template <typename T>
 struct Tma2gCtx final : lbwp_ctx {
     lbwp::Tma2gPlanBase* planp = nullptr;
     lbwp::XLayout X;
+    int sms = 148;
     ~Tma2gCtx() override { delete planp; }
 
     int prepare() {
@@ -349,6 +351,12 @@ struct Tma2gCtx final : lbwp_ctx {
         if (!planp) return fail(LBWP_ENOMEM, "no fused two-component TMA plan");
         int rc = planp->setup(X, buf);
         if (rc) return fail(rc < 0 ? LBWP_EUNSUPPORTED : LBWP_ECUDA, "fused two-component TMA plan setup failed (%d)", rc);
+        if (P.A_h != 0.0) {   // min and max of rA per box, written by k_contact_scan (the layout's box grid is the same for both buffers)
+            cudaError_t e = cudaMalloc(&grad, (size_t)2 * lbwp::contact_boxes(X).count() * sizeof(T));
+            if (e != cudaSuccess) return fail(LBWP_ENOMEM, "cudaMalloc(near-contact box ranges): %s", cudaGetErrorString(e));
+            e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, P.device);
+            if (e != cudaSuccess) return fail(LBWP_ECUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e));
+        }
         return LBWP_OK;
     }
     // near-contact force (lbwp_contact.cuh): Guo's forcing applied to the collided moments of buffer b, in place
@@ -357,9 +365,18 @@ struct Tma2gCtx final : lbwp_ctx {
         lbwp::ContactParams<T> cp;
         cp.L = planp->Lb[b]; cp.state = (T*)buf[b];
         cp.omega = T(1.0 / P.tau); cp.A_h = T(P.A_h); cp.h_c = T(P.h_c);
-        const dim3 blk(32, 8, 1), g((X.nx + 31) / 32, (X.ny + 7) / 8, X.nz);
-        if (P.lattice == 27) lbwp::k_contact_fixup<T, 27><<<g, blk, 0, stream>>>(cp);
-        else lbwp::k_contact_fixup<T, 19><<<g, blk, 0, stream>>>(cp);
+        using namespace lbwp;
+        const ContactBoxes B = contact_boxes(cp.L);
+        const dim3 blk(CONTACT_BX, CONTACT_BY, 1);
+        const T* ra = (const T*)buf[b] + 10 * cp.L.field;
+        const int zb = B.count() >= 64 * sms ? 8 : 2;           // boxes along z per CTA of the scan
+        const dim3 gs(B.nbx, B.nby, (B.nbz + zb - 1) / zb);
+        if (zb == 8) k_contact_scan<T, 8><<<gs, blk, 0, stream>>>(cp.L, B, ra, (T*)grad);
+        else k_contact_scan<T, 2><<<gs, blk, 0, stream>>>(cp.L, B, ra, (T*)grad);
+        const int split = B.count() >= 64 * sms ? 1 : CONTACT_BZ;   // 128^3: 2048 boxes, 512^3: 131072
+        const int gf = (int)std::min<long long>((long long)B.count() * split, 8 * sms);
+        if (P.lattice == 27) k_contact_fixup<T, 27><<<gf, blk, 0, stream>>>(cp, B, (const T*)grad, split);
+        else k_contact_fixup<T, 19><<<gf, blk, 0, stream>>>(cp, B, (const T*)grad, split);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return fail(LBWP_ECUDA, "near-contact fix-up launch: %s", cudaGetErrorString(e));
         return LBWP_OK;
@@ -508,7 +525,7 @@ int lbwp_init(const lbwp_params* p, const void* moments, int moments_on_device, 
     if (variant == LBWP_KERNEL_TMA) {
         if (tma2_fused(p)) {
             rc = p->dtype == LBWP_F32 ? static_cast<Tma2gCtx<float>*>(c)->prepare() : static_cast<Tma2gCtx<double>*>(c)->prepare();
-            c->launches_per_step = p->A_h != 0.0 ? 2 : 1;   // + the near-contact fix-up pass
+            c->launches_per_step = p->A_h != 0.0 ? 3 : 1;   // + the two kernels of the near-contact fix-up pass
         } else if (p->ncomp == 2) {
             rc = p->dtype == LBWP_F32 ? static_cast<Tma2Ctx<float>*>(c)->prepare() : static_cast<Tma2Ctx<double>*>(c)->prepare();
             c->launches_per_step = 2;

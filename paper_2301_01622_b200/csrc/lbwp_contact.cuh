@@ -15,8 +15,9 @@
 //        J += 3 F,  Sd_a += 4.5 dS_aa,  So_ab += 9 dS_ab,  a -= 1.5 tr dS            (all x the state's scale),
 //      with rho, u = j / rho recovered from the S-form itself.
 // Only rA is read at other nodes and only the fields 0..9 of the own node are written, so the pass is race-free in
-// place.  Traffic: rA once per node (its 27 neighbours come from L1/L2) and ten fields read + written at the few
-// nodes of a film between two interfaces: about 5 % of the step's.
+// place.  Traffic: rA once per node (a CTA whose box and halo lie in one bulk phase leaves after reading them; elsewhere
+// the 27 neighbours come from L1/L2) and ten fields read + written at the few nodes of a film between two interfaces:
+// about 5 % of the step's.
 #pragma once
 #include "lbwp_tma.cuh"
 
@@ -55,13 +56,10 @@ __device__ __forceinline__ void contact_gradient(const XLayout& L, const T* __re
     gx *= T(6); gy *= T(6); gz *= T(6);
 }
 
+// steps 1-3 at one node
 template <typename T, int Q>
-__global__ void __launch_bounds__(256) k_contact_fixup(const ContactParams<T> p) {
-    const int x = blockIdx.x * blockDim.x + threadIdx.x;
-    const int y = blockIdx.y * blockDim.y + threadIdx.y;
-    const int z = blockIdx.z;
+__device__ __forceinline__ void contact_node(const ContactParams<T>& p, int x, int y, int z) {
     const XLayout& L = p.L;
-    if (x >= L.nx || y >= L.ny) return;
     const long long F = L.field;
     const T* __restrict__ ra = p.state + 10 * F;
     T gx, gy, gz;
@@ -121,6 +119,133 @@ __global__ void __launch_bounds__(256) k_contact_fixup(const ContactParams<T> p)
         T* __restrict__ g = x < 3 ? d + L.nx : d - L.nx;
 #pragma unroll
         for (int f = 0; f < 10; ++f) g[f * F] = s[f];
+    }
+}
+
+// The force acts on the few nodes of a film between two interfaces; everywhere else step 2 leaves at once.  Two kernels
+// keep the pass from paying 26 loads per node for that:
+//   k_contact_scan   reads rA once, coalesced, and stores min and max of rA over every box of CONTACT_BX x CONTACT_BY x
+//                    CONTACT_BZ nodes (range[0][box], range[1][box]; the last boxes may overhang the grid);
+//   k_contact_fixup  a persistent kernel (its CTAs share the boxes out round-robin): for every box it takes min and max over the box and its 26 neighbours (which
+//                    cover the box's halo of one node, periodic).  G_a = 6 (sum_{c_ia = +1} w_i rA_i - sum_{c_ia = -1}
+//                    w_i rA_i) and sum_{c_ia = +1} w_i = 1/6 on both lattices, so |G_a| <= max - min and |G|^2 <=
+//                    3 (max - min)^2: where max - min < 0.02 every node of the box has |G|^2 <= 1.2e-3 < G_I^2 = 2.5e-3
+//                    and the box is skipped (exact: no node that gets a force is skipped).  The CTA runs steps 1-3 on
+//                    the nodes of the remaining boxes.
+constexpr int CONTACT_BX = 32, CONTACT_BY = 8, CONTACT_BZ = 4;
+constexpr int CONTACT_CH = 32;    // boxes classified per round of a fix-up CTA
+
+struct ContactBoxes {
+    int nbx, nby, nbz;
+    __host__ __device__ int count() const { return nbx * nby * nbz; }
+};
+inline ContactBoxes contact_boxes(const XLayout& L) {
+    return {(L.nx + CONTACT_BX - 1) / CONTACT_BX, (L.ny + CONTACT_BY - 1) / CONTACT_BY, (L.nz + CONTACT_BZ - 1) / CONTACT_BZ};
+}
+
+// ZB: boxes along z per CTA (8 on large grids, 2 where that would leave fewer CTAs than the GPU holds)
+template <typename T, int ZB>
+__global__ void __launch_bounds__(CONTACT_BX * CONTACT_BY) k_contact_scan(const XLayout L, const ContactBoxes B, const T* __restrict__ ra,
+                                                                          T* __restrict__ range) {
+    constexpr int NW = CONTACT_BX * CONTACT_BY / 32;
+    __shared__ T s_lo[ZB][NW], s_hi[ZB][NW];
+    const int tid = threadIdx.y * CONTACT_BX + threadIdx.x;
+    int x = blockIdx.x * CONTACT_BX + threadIdx.x, y = blockIdx.y * CONTACT_BY + threadIdx.y;
+    x = x < L.nx ? x : L.nx - 1;                               // a repeated node changes neither min nor max
+    y = y < L.ny ? y : L.ny - 1;
+    const int bz0 = blockIdx.z * ZB;
+#pragma unroll
+    for (int k = 0; k < ZB; ++k) {
+        if (bz0 + k >= B.nbz) break;
+        T v[CONTACT_BZ];
+#pragma unroll
+        for (int j = 0; j < CONTACT_BZ; ++j) {
+            int z = (bz0 + k) * CONTACT_BZ + j;
+            z = z < L.nz ? z : L.nz - 1;
+            v[j] = ra[xidx(L, x, y, z)];
+        }
+        T lo = v[0], hi = v[0];
+#pragma unroll
+        for (int j = 1; j < CONTACT_BZ; ++j) {
+            lo = v[j] < lo ? v[j] : lo;
+            hi = v[j] > hi ? v[j] : hi;
+        }
+#pragma unroll
+        for (int o = 16; o; o >>= 1) {
+            const T a = __shfl_xor_sync(0xffffffffu, lo, o), b = __shfl_xor_sync(0xffffffffu, hi, o);
+            lo = a < lo ? a : lo;
+            hi = b > hi ? b : hi;
+        }
+        if ((tid & 31) == 0) { s_lo[k][tid >> 5] = lo; s_hi[k][tid >> 5] = hi; }
+    }
+    __syncthreads();
+    if (tid < ZB && bz0 + tid < B.nbz) {
+        T lo = s_lo[tid][0], hi = s_hi[tid][0];
+#pragma unroll
+        for (int w = 1; w < NW; ++w) {
+            lo = s_lo[tid][w] < lo ? s_lo[tid][w] : lo;
+            hi = s_hi[tid][w] > hi ? s_hi[tid][w] : hi;
+        }
+        const int box = ((bz0 + tid) * B.nby + blockIdx.y) * B.nbx + blockIdx.x;
+        range[box] = lo;
+        range[B.count() + box] = hi;
+    }
+}
+
+template <typename T, int Q>
+__global__ void __launch_bounds__(CONTACT_BX * CONTACT_BY, sizeof(T) == 4 ? 4 : 2) k_contact_fixup(const ContactParams<T> p, const ContactBoxes B,
+                                                                           const T* __restrict__ range, const int split) {
+    constexpr int NT = CONTACT_BX * CONTACT_BY, SUB = NT / CONTACT_CH;   // SUB threads share the 27 neighbours of a box
+    static_assert(SUB == 8, "the reduction below runs over 8 adjacent lanes");
+    __shared__ int s_list[CONTACT_CH];
+    __shared__ int s_n;
+    const XLayout& L = p.L;
+    const int tid = threadIdx.y * CONTACT_BX + threadIdx.x;
+    const int nbox = B.count();
+    // An item is a box's planes part * BZ / split ... (split = 1, 2 or 4: on a small grid the planes of a box go to
+    // different CTAs, there are not enough boxes to fill the GPU otherwise).  CTA b of G takes the items b, b + G,
+    // b + 2 G, ...: the boxes of an interface are neighbours in the box grid, this spreads them over all CTAs.
+    const long long nitem = (long long)nbox * split;
+    for (long long first = 0; first + blockIdx.x < nitem; first += (long long)CONTACT_CH * gridDim.x) {
+        if (tid == 0) s_n = 0;
+        __syncthreads();
+        const long long id = first + (long long)(tid / SUB) * gridDim.x + blockIdx.x;
+        const int item = id < nitem ? (int)id : -1, box = item < 0 ? nbox : item / split, sub = tid % SUB;
+        T lo = T(1e30), hi = T(-1e30);
+        if (box < nbox) {
+            const int bx = box % B.nbx, by = (box / B.nbx) % B.nby, bz = box / (B.nbx * B.nby);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int nb = sub + k * SUB;
+                if (nb < 27) {
+                    int qx = bx + nb % 3 - 1, qy = by + (nb / 3) % 3 - 1, qz = bz + nb / 9 - 1;
+                    qx = qx < 0 ? B.nbx - 1 : qx == B.nbx ? 0 : qx;
+                    qy = qy < 0 ? B.nby - 1 : qy == B.nby ? 0 : qy;
+                    qz = qz < 0 ? B.nbz - 1 : qz == B.nbz ? 0 : qz;
+                    const int q = (qz * B.nby + qy) * B.nbx + qx;
+                    const T a = range[q], b = range[nbox + q];
+                    lo = a < lo ? a : lo;
+                    hi = b > hi ? b : hi;
+                }
+            }
+        }
+#pragma unroll
+        for (int o = 1; o < SUB; o <<= 1) {
+            const T a = __shfl_xor_sync(0xffffffffu, lo, o), b = __shfl_xor_sync(0xffffffffu, hi, o);
+            lo = a < lo ? a : lo;
+            hi = b > hi ? b : hi;
+        }
+        if (sub == 0 && box < nbox && !(hi - lo < T(0.02))) s_list[atomicAdd(&s_n, 1)] = item;
+        __syncthreads();
+        const int n = s_n;
+        for (int k = 0; k < n; ++k) {
+            const int b = s_list[k] / split, part = s_list[k] % split;
+            const int x = (b % B.nbx) * CONTACT_BX + threadIdx.x, y = ((b / B.nbx) % B.nby) * CONTACT_BY + threadIdx.y;
+            const int z0 = (b / (B.nbx * B.nby)) * CONTACT_BZ + part * (CONTACT_BZ / split), z1 = z0 + CONTACT_BZ / split;
+            if (x < L.nx && y < L.ny)
+                for (int z = z0; z < z1 && z < L.nz; ++z) contact_node<T, Q>(p, x, y, z);
+        }
+        __syncthreads();
     }
 }
 

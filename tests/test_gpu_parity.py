@@ -353,10 +353,13 @@ def test_near_contact_force(lbwp, oracle, dtype, lattice):
 
 # the same force behind the fused two-component TMA kernel (a fix-up pass on the collided moments, lbwp_contact.cuh):
 # a box the tiles divide, the drops pressed against each other across tile, chunk and periodic boundaries
+# nz = 38: the fix-up pass's boxes of four planes overhang the grid; h_c = 6: its walk leaves the shared-memory tile, so
+# the kernel variant that reads rA from global memory runs
+@pytest.mark.parametrize("nz,h_c", [(36, 4.0), (38, 4.0), (36, 6.0)])
 @pytest.mark.parametrize("lattice", [19, 27])
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
-def test_near_contact_force_fused(lbwp, oracle, dtype, lattice):
-    shape = (64, 40, 36)
+def test_near_contact_force_fused(lbwp, oracle, dtype, lattice, nz, h_c):
+    shape = (64, 40, nz)
     nx, ny, nz = shape
     R, gap = 9.0, 2.0
     d = 2 * R + gap
@@ -366,21 +369,21 @@ def test_near_contact_force_fused(lbwp, oracle, dtype, lattice):
     m0 = wl.as_dtype(m, dtype)
     kw = dict(lattice=lattice, tau=0.8, A=0.01, beta=0.7)
     steps = 25
-    with lbwp.Lbwp(m0, dtype=dtype, ncomp=2, A_h=0.02, h_c=4.0, **kw) as sim:
-        assert sim.kernel_name == "tma%d_%s_c2" % (lattice, dtype) and sim.launches_per_step == 2
+    with lbwp.Lbwp(m0, dtype=dtype, ncomp=2, A_h=0.02, h_c=h_c, **kw) as sim:
+        assert sim.kernel_name == "tma%d_%s_c2" % (lattice, dtype) and sim.launches_per_step == 3
         sim.step(steps)
         got = sim.moments_host()
         sim.step(1)                                          # lbwp_moments after a further step: the export path
         got1 = sim.moments_host()
-    ref = oracle.run_nc(m0, nsteps=steps, A_h=0.02, h_c=4.0, **kw)
+    ref = oracle.run_nc(m0, nsteps=steps, A_h=0.02, h_c=h_c, **kw)
     errs, _ = report("near_contact_fused_q%d/%s/%d steps" % (lattice, dtype, steps), got, ref, 2, dtype)
     assert errs.max() <= TOL[dtype], errs
     assert sign_agreement(got, ref) >= 0.9999
-    ref1 = oracle.run_nc(ref, nsteps=1, A_h=0.02, h_c=4.0, **kw)
+    ref1 = oracle.run_nc(ref, nsteps=1, A_h=0.02, h_c=h_c, **kw)
     assert parity_errors(got1, ref1, 2, dtype).max() <= TOL[dtype]
     off = oracle.run(m0, ncomp=2, nsteps=steps, **kw)
     assert np.abs(ref - off).max() > 1e-3                    # the repulsion changed the collision
-    with lbwp.Lbwp(m0, dtype=dtype, ncomp=2, A_h=0.02, h_c=4.0, kernel="gather", **kw) as sim:   # and the generic path agrees
+    with lbwp.Lbwp(m0, dtype=dtype, ncomp=2, A_h=0.02, h_c=h_c, kernel="gather", **kw) as sim:   # and the generic path agrees
         sim.step(steps)
         gen = sim.moments_host()
     assert parity_errors(got, gen.astype(np.float64), 2, dtype).max() <= TOL[dtype]
