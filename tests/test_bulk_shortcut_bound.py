@@ -53,3 +53,30 @@ def test_gradient_bound_in_a_bulk_neighbourhood(q, bulk):
     # the same sums in fp32 (the kernel's arithmetic, any order): rounding of values near 1 moves |G|^2 by far less
     G32 = 6 * np.einsum("i,ia,ni->na", w.astype(np.float32), c.astype(np.float32), (bulk + d).astype(np.float32))
     assert (G32.astype(np.float64) ** 2).sum(1).max() < G2CUT
+
+
+# ---- the near-contact fix-up pass (csrc/lbwp_contact.cuh) skips a box of nodes when rA over the
+#      box and its halo of one node spans less than SPAN: then |G_a| <= max - min at every node of the box (the weights
+#      of the directions with c_ia = +1 sum to 1/6) and |G|^2 <= 3 SPAN^2 stays below G_I^2 (reading C22), so no node of
+#      the box would start the interface walk ------------------------------------------------------------------------
+SPAN = 0.02           # the cut of k_contact_fixup
+GI2 = 0.05 ** 2       # G_I^2 (reading C22)
+
+
+@pytest.mark.parametrize("q", [19, 27])
+def test_contact_box_skip_bound(q):
+    c, w = lattice(q)
+    for a in range(3):
+        assert abs(w[c[:, a] > 0].sum() - 1 / 6) < 1e-15 and abs(w[c[:, a] < 0].sum() - 1 / 6) < 1e-15
+    assert 3 * SPAN ** 2 < GI2 / 2                                    # factor-two margin
+    rng = np.random.default_rng(11)
+    lo = rng.uniform(0, 1 - SPAN, (20000, 1))
+    r = lo + rng.uniform(0, SPAN, (20000, len(w)))                    # any field of that span, not only near a bulk value
+    r[:, :2] = np.stack([lo[:, 0], lo[:, 0] + SPAN], 1)               # the extremes are attained
+    G = 6 * np.einsum("i,ia,ni->na", w, c, r)
+    span = r.max(1) - r.min(1)
+    assert (np.abs(G).max(1) <= span + 1e-15).all()
+    worst = np.where(c[:, 0] > 0, SPAN, 0.0)                          # maximises G_x: 6 SPAN / 6 = SPAN
+    assert abs(6 * (w * c[:, 0] * worst).sum() - SPAN) < 1e-15
+    G32 = 6 * np.einsum("i,ia,ni->na", w.astype(np.float32), c.astype(np.float32), r.astype(np.float32))
+    assert (G32.astype(np.float64) ** 2).sum(1).max() < GI2
