@@ -277,11 +277,12 @@ def main():
         # field is the n^3 recipe repeated along z, so each rank's halo-extended slab is cut from its own copy.
         from paper_2301_01622_b200 import slabs
         cfg = wl.sweep_case(a.n, a.lattice, a.ncomp, a.dtype)
-        halo = slabs.halo_width(a.ncomp)
+        A_h = a.near_contact if a.ncomp == 2 else 0.0
+        halo = slabs.halo_width(a.ncomp, A_h)
         m0 = wl.as_dtype(cfg["moments"], a.dtype)
         m0 = np.ascontiguousarray(m0[:, np.arange(-halo, a.n + halo) % a.n])
         slab = slabs.SlabLbwp(m0, world=world, rank=rank, lattice=a.lattice, dtype=a.dtype, ncomp=a.ncomp, tau=cfg["tau"],
-                              A=cfg["A"], beta=cfg["beta"], kernel=a.kernel, device=local)
+                              A=cfg["A"], beta=cfg["beta"], kernel=a.kernel, device=local, A_h=A_h)
         sim = slab.sim
         stepper = slab
     else:

@@ -78,12 +78,13 @@ typedef struct lbwp_params {
     double A_h;          /* ncomp == 2, moments scheme: strength of the near-contact repulsion
                             F_rep = -A_h[h(x)] n delta_I (Eq. 10; readings C20-C24 of DESIGN.md:
                             delta_I = |grad phi|/2, n the outward normal, A_h[h] = A_h for h <= h_c and 0 beyond,
-                            Guo forcing).  0 = off (BASELINE's configs).  Non-zero adds a second launch per step behind
-                            the fused two-component TMA kernel (a pointwise pass that finds the facing interfaces
-                            and applies the forcing to the collided moments in place), or, for boxes the TMA tiles
-                            do not divide and with LBWP_KERNEL_GATHER, selects the generic kernel (three launches
-                            per step: gradient, contact search, step); LBWP_EUNSUPPORTED with LBWP_KERNEL_TMA_SPLIT /
-                            MARCH and in the lbwp_halo_* calls (the force looks h_c + 1 planes beyond a node). */
+                            Guo forcing).  0 = off (BASELINE's configs).  Non-zero adds two launches per step behind
+                            the fused two-component TMA kernel (min / max of rA per box of nodes, then a pass over
+                            the boxes that hold an interface: it finds the facing interfaces and applies the forcing
+                            to the collided moments in place), or, for boxes the TMA tiles do not divide and with
+                            LBWP_KERNEL_GATHER, selects the generic kernel (three launches per step: gradient,
+                            contact search, step); LBWP_EUNSUPPORTED with LBWP_KERNEL_TMA_SPLIT / MARCH.  The force
+                            looks floor(h_c) + 1 planes beyond a node: slabs then need H = floor(h_c) + 3 halo planes. */
     double h_c;          /* cut-off distance of the near-contact force in lattice units (> 0 when A_h != 0) */
 } lbwp_params;
 
@@ -171,7 +172,8 @@ int lbwp_diagnostics_static(int device, int dtype, int ncomp, int nx, int ny, in
 /* z-slab decomposition over several GPUs (the paper's motivation are grids of billions of nodes,
  * PAPER.md:163-167).  A rank's context is an ordinary periodic box whose first and last H planes are HALO planes:
  * copies of the neighbouring ranks' boundary planes (H = 1; H = 2 for ncomp == 2 moments, whose colour gradient
- * reaches two planes).  One step of the decomposed box = lbwp_step(ctx, 1) on every rank, then every rank packs its
+ * reaches two planes; H = floor(h_c) + 3 with the near-contact force, whose interface walk and the gradients on its
+ * way reach floor(h_c) + 1 planes beyond the two the step leaves wrong).  One step of the decomposed box = lbwp_step(ctx, 1) on every rank, then every rank packs its
  * H lowest and H highest OWNED planes of the new state, sends them to its z neighbours (NCCL send/recv, or a peer
  * copy) and unpacks what it receives into its halo planes.  The planes the step computed INTO the halo are garbage
  * (the box wrapped onto itself there) and are overwritten by the unpack.  The packed format is the library's private

@@ -682,7 +682,6 @@ namespace {
 int halo_copy(lbwp_ctx* c, int z0, int nplanes, void* packed, bool pack) {
     if (!c || !packed) return fail(LBWP_EINVAL, "lbwp_halo_*: NULL argument");
     if (c->P.scheme != LBWP_MOMENTS) return fail(LBWP_EUNSUPPORTED, "lbwp_halo_*: moments scheme only");
-    if (c->P.A_h != 0.0) return fail(LBWP_EUNSUPPORTED, "lbwp_halo_*: the near-contact force reaches h_c + 1 planes, more than the halo carries");
     if (nplanes < 1 || z0 < 0 || z0 + nplanes > c->L.nz) return fail(LBWP_EINVAL, "lbwp_halo_*: planes [%d, %d) leave the box", z0, z0 + nplanes);
     DeviceGuard guard(c->P.device);
     if (!guard.ok) return fail(LBWP_ECUDA, "cudaSetDevice(%d) failed", c->P.device);

@@ -10,7 +10,7 @@ on each side, as an ordinary periodic box of the library (``lbwp_ctx``).  One ti
     lbwp_halo_unpack x 2                   into the halo planes
 
 H = 1 (the stencil reaches one plane), H = 2 for two-component moments (the colour gradient of a source plane reaches
-one plane further).  Everything the method computes runs inside the library's kernels; this module only moves opaque
+one plane further), H = floor(h_c) + 3 with the near-contact force (its interface walk and the gradients on the way).  Everything the method computes runs inside the library's kernels; this module only moves opaque
 packed planes between ranks (marshalling and communication plumbing).  Per face and step the exchange carries
 ``M * nx * ny * sizeof`` bytes (10.6 MB at 512^2 fp32): about 12 us at NVLink 5 rates against a step of 1-2 ms.
 """
@@ -19,9 +19,17 @@ from __future__ import annotations
 import numpy as np
 
 
-def halo_width(ncomp: int) -> int:
-    """Halo planes a slab needs on each side (moments scheme)."""
+def halo_width(ncomp: int, A_h: float = 0.0, h_c: float = 4.0) -> int:
+    """Halo planes a slab needs on each side (moments scheme).  With the near-contact force a node's
+    force looks floor(h_c) + 1 planes away (the interface walk, plus the gradient at the node it stops on), on top of
+    the 2 outermost planes a step leaves wrong."""
+    if ncomp == 2 and A_h:
+        return 2 + int(np.floor(h_c)) + 1
     return 2 if ncomp == 2 else 1
+
+
+def _halo_of(kw: dict) -> int:
+    return halo_width(kw.get("ncomp", 1), kw.get("A_h", 0.0), kw.get("h_c", 4.0))
 
 
 def slab_range(nz: int, world: int, rank: int):
@@ -100,12 +108,9 @@ class SlabLbwp:
         from . import lbwp
 
         self.world, self.rank = world, rank
-        self.halo = halo_width(lbwp_kwargs.get("ncomp", 1))
+        self.halo = _halo_of(lbwp_kwargs)
         if lbwp_kwargs.get("scheme", "moments") != "moments":
             raise ValueError("slab decomposition: moments scheme only")
-        if lbwp_kwargs.get("A_h", 0.0):
-            raise ValueError("slab decomposition: the near-contact force looks h_c + 1 planes beyond a node "
-                             "(interface walk plus gradient), more than the halo carries; not supported")
         self.sim = lbwp.Lbwp(local_m0, **lbwp_kwargs)
         self.nz_local = self.sim.shape[0]
         self.owned = self.nz_local - 2 * self.halo
@@ -153,7 +158,7 @@ class SlabGroup:
     def __init__(self, global_m0, world, **lbwp_kwargs):
         self.world = world
         self.mailbox = {}
-        halo = halo_width(lbwp_kwargs.get("ncomp", 1))
+        halo = _halo_of(lbwp_kwargs)
         self.slabs = [SlabLbwp(local_moments(global_m0, world, r, halo), world=world, rank=r,
                                transport=LocalTransport(world, r, self.mailbox), **lbwp_kwargs) for r in range(world)]
 

@@ -34,6 +34,8 @@ def test_local_planes_wrap():
     assert slabs.local_planes(10, 3, 0, 1).tolist() == [9, 0, 1, 2, 3, 4]        # lower halo wraps to the top of the box
     assert slabs.local_planes(10, 3, 2, 2).tolist() == [5, 6, 7, 8, 9, 0, 1]     # upper halo wraps to the bottom
     assert slabs.halo_width(1) == 1 and slabs.halo_width(2) == 2
+    assert slabs.halo_width(2, A_h=0.02, h_c=4.0) == 7 and slabs.halo_width(2, A_h=0.02, h_c=2.5) == 5   # near-contact walk
+    assert slabs.halo_width(1, A_h=0.02) == 1
     g = np.arange(2 * 10 * 1 * 1, dtype=np.float64).reshape(2, 10, 1, 1)
     loc = slabs.local_moments(g, 3, 1, 1)
     assert loc.shape == (2, 5, 1, 1) and loc[0, :, 0, 0].tolist() == [3, 4, 5, 6, 7]
@@ -43,8 +45,6 @@ def test_local_planes_wrap():
 
 def test_slab_rejects_what_the_halo_cannot_carry():
     m = np.zeros((11, 8, 8, 64), dtype=np.float32)
-    with pytest.raises(ValueError, match="near-contact"):
-        slabs.SlabLbwp(m, world=2, rank=0, ncomp=2, tau=1.0, A=0.01, beta=0.7, A_h=0.01)
     with pytest.raises(ValueError, match="moments scheme"):
         slabs.SlabLbwp(m, world=2, rank=0, ncomp=2, tau=1.0, scheme="populations")
 
@@ -74,7 +74,7 @@ def _stencil_worker(rank, world, port, nz, halo, steps, out):
     dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("world,nz,halo", [(2, 9, 1), (3, 10, 2), (2, 8, 2)])
+@pytest.mark.parametrize("world,nz,halo", [(2, 9, 1), (3, 10, 2), (2, 8, 2), (2, 29, 7)])   # 7: the near-contact halo
 def test_exchange_over_gloo(world, nz, halo):
     steps = 5
     ctx = mp.get_context("spawn")
@@ -130,6 +130,43 @@ def test_slabs_equal_single_box(world, ncomp, dtype, shape, lattice):
     finally:
         grp.close()
     assert parts.shape == whole.shape
+    assert np.array_equal(parts, whole), float(np.abs(parts.astype(np.float64) - whole).max())
+
+
+# the near-contact force in slabs (halo floor(h_c) + 3 = 7 planes): two drops pressed against each other, the film between
+# them lying across the slab boundary; the fused path (fix-up pass behind the TMA kernel) and the generic one
+@pytest.mark.gpu
+@pytest.mark.parametrize("dtype,shape,lattice,kernel", [("f32", (64, 40, 36), 19, "tma"), ("f64", (64, 40, 37), 27, "tma"),
+                                                        ("f32", (40, 36, 34), 27, "gather")])
+def test_slabs_near_contact_equal_single_box(dtype, shape, lattice, kernel):
+    from paper_2301_01622_b200 import build as lbuild
+    from paper_2301_01622_b200 import lbwp
+    lbuild.build()
+    nx, ny, nz = shape
+    R, gap = 9.0, 2.0
+    d = 2 * R + gap
+    # the drops face each other along z, the film at z = nz / 2: the boundary between the two slabs
+    uz = np.broadcast_to(0.03 * np.cos(2 * np.pi * (np.arange(nz) + 0.5) / nz)[:, None, None], (nz, ny, nx))   # a flow along z, through the slab boundaries
+    m = wl.droplets(0, [(nx / 2 - 2, ny / 2, nz / 2 - d / 2), (nx / 2 + 2, ny / 2, nz / 2 + d / 2)], R, [0.0, 0.0],
+                    background_u=[np.zeros((nz, ny, nx)), np.zeros((nz, ny, nx)), uz], shape=shape)
+    m0 = wl.as_dtype(m, dtype)
+    kw = dict(lattice=lattice, dtype=dtype, ncomp=2, tau=0.8, A=0.01, beta=0.7, A_h=0.02, h_c=4.0)
+    steps = 15
+    with lbwp.Lbwp(m0, **kw) as sim:
+        assert sim.kernel_name.startswith(kernel)
+        sim.step(steps)
+        whole = sim.moments_host()
+        name = sim.kernel_name
+    with lbwp.Lbwp(m0, **dict(kw, A_h=0.0)) as sim:
+        sim.step(steps)
+        assert np.abs(sim.moments_host().astype(np.float64) - whole).max() > 1e-4   # the force acts in this set-up
+    grp = slabs.SlabGroup(m0, 2, **kw)
+    try:
+        assert all(s.sim.kernel_name == name and s.halo == 7 for s in grp.slabs)
+        grp.step(steps)
+        parts = grp.moments()
+    finally:
+        grp.close()
     assert np.array_equal(parts, whole), float(np.abs(parts.astype(np.float64) - whole).max())
 
 
