@@ -77,13 +77,19 @@ __device__ __forceinline__ void contact_node(const ContactParams<T>& p, int x, i
                 const int n2 = cx * cx + cy * cy + cz * cz;
                 if (n2 == 0 || (Q == 19 && n2 == 3)) continue;
                 const T norm = n2 == 1 ? T(1) : n2 == 2 ? T(1.4142135623730951) : T(1.7320508075688772);
-                const T cosv = -(T(cx) * gx + T(cy) * gy + T(cz) * gz) / norm;
+                const T inorm = n2 == 1 ? T(1) : n2 == 2 ? T(0.7071067811865476) : T(0.5773502691896258);
+                const T cosv = -(T(cx) * gx + T(cy) * gy + T(cz) * gz) * inorm;   // directions that mirror each other tie exactly
                 if (cosv > best) { best = cosv; mx = cx; my = cy; mz = cz; len = norm; }
             }
     bool facing = false;
     for (int k = 1; T(k) * len <= p.h_c && !facing; ++k) {
-        int px = (x + k * mx) % L.nx, py = (y + k * my) % L.ny, pz = (z + k * mz) % L.nz;   // periodic (reading C13)
-        px += px < 0 ? L.nx : 0; py += py < 0 ? L.ny : 0; pz += pz < 0 ? L.nz : 0;
+        int px = x + k * mx, py = y + k * my, pz = z + k * mz;                               // periodic (reading C13)
+        while (px < 0) px += L.nx;
+        while (px >= L.nx) px -= L.nx;
+        while (py < 0) py += L.ny;
+        while (py >= L.ny) py -= L.ny;
+        while (pz < 0) pz += L.nz;
+        while (pz >= L.nz) pz -= L.nz;
         T qx, qy, qz;
         contact_gradient<T, Q>(L, ra, px, py, pz, qx, qy, qz);
         facing = qx * qx + qy * qy + qz * qz > GI2 && qx * gx + qy * gy + qz * gz < T(0);
@@ -143,6 +149,23 @@ inline ContactBoxes contact_boxes(const XLayout& L) {
     return {(L.nx + CONTACT_BX - 1) / CONTACT_BX, (L.ny + CONTACT_BY - 1) / CONTACT_BY, (L.nz + CONTACT_BZ - 1) / CONTACT_BZ};
 }
 
+// min and max over the lanes of a warp (to every lane).  fp32 goes through the integer warp reduction (redux.sync): the
+// bit pattern of a float, with the low 31 bits flipped when negative, orders as a signed integer like the float does.
+__device__ __forceinline__ int contact_ord(float f) { const int i = __float_as_int(f); return i ^ ((i >> 31) & 0x7fffffff); }
+__device__ __forceinline__ float contact_unord(int i) { return __int_as_float(i ^ ((i >> 31) & 0x7fffffff)); }
+__device__ __forceinline__ void contact_warp_range(float& lo, float& hi) {
+    lo = contact_unord(__reduce_min_sync(0xffffffffu, contact_ord(lo)));
+    hi = contact_unord(__reduce_max_sync(0xffffffffu, contact_ord(hi)));
+}
+__device__ __forceinline__ void contact_warp_range(double& lo, double& hi) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+        const double a = __shfl_xor_sync(0xffffffffu, lo, o), b = __shfl_xor_sync(0xffffffffu, hi, o);
+        lo = a < lo ? a : lo;
+        hi = b > hi ? b : hi;
+    }
+}
+
 // ZB: boxes along z per CTA (8 on large grids, 2 where that would leave fewer CTAs than the GPU holds)
 template <typename T, int ZB>
 __global__ void __launch_bounds__(CONTACT_BX * CONTACT_BY) k_contact_scan(const XLayout L, const ContactBoxes B, const T* __restrict__ ra,
@@ -170,12 +193,7 @@ __global__ void __launch_bounds__(CONTACT_BX * CONTACT_BY) k_contact_scan(const 
             lo = v[j] < lo ? v[j] : lo;
             hi = v[j] > hi ? v[j] : hi;
         }
-#pragma unroll
-        for (int o = 16; o; o >>= 1) {
-            const T a = __shfl_xor_sync(0xffffffffu, lo, o), b = __shfl_xor_sync(0xffffffffu, hi, o);
-            lo = a < lo ? a : lo;
-            hi = b > hi ? b : hi;
-        }
+        contact_warp_range(lo, hi);
         if ((tid & 31) == 0) { s_lo[k][tid >> 5] = lo; s_hi[k][tid >> 5] = hi; }
     }
     __syncthreads();
@@ -197,7 +215,7 @@ __global__ void __launch_bounds__(CONTACT_BX * CONTACT_BY, sizeof(T) == 4 ? 4 : 
                                                                            const T* __restrict__ range, const int split) {
     constexpr int NT = CONTACT_BX * CONTACT_BY, SUB = NT / CONTACT_CH;   // SUB threads share the 27 neighbours of a box
     static_assert(SUB == 8, "the reduction below runs over 8 adjacent lanes");
-    __shared__ int s_list[CONTACT_CH];
+    __shared__ int4 s_list[CONTACT_CH];   // x0, y0, z0, z1 of the items to work on
     __shared__ int s_n;
     const XLayout& L = p.L;
     const int tid = threadIdx.y * CONTACT_BX + threadIdx.x;
@@ -212,8 +230,9 @@ __global__ void __launch_bounds__(CONTACT_BX * CONTACT_BY, sizeof(T) == 4 ? 4 : 
         const long long id = first + (long long)(tid / SUB) * gridDim.x + blockIdx.x;
         const int item = id < nitem ? (int)id : -1, box = item < 0 ? nbox : item / split, sub = tid % SUB;
         T lo = T(1e30), hi = T(-1e30);
+        int bx = 0, by = 0, bz = 0;
         if (box < nbox) {
-            const int bx = box % B.nbx, by = (box / B.nbx) % B.nby, bz = box / (B.nbx * B.nby);
+            bx = box % B.nbx; by = (box / B.nbx) % B.nby; bz = box / (B.nbx * B.nby);
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
                 const int nb = sub + k * SUB;
@@ -235,15 +254,17 @@ __global__ void __launch_bounds__(CONTACT_BX * CONTACT_BY, sizeof(T) == 4 ? 4 : 
             lo = a < lo ? a : lo;
             hi = b > hi ? b : hi;
         }
-        if (sub == 0 && box < nbox && !(hi - lo < T(0.02))) s_list[atomicAdd(&s_n, 1)] = item;
+        if (sub == 0 && box < nbox && !(hi - lo < T(0.02))) {
+            const int z0 = bz * CONTACT_BZ + (item % split) * (CONTACT_BZ / split);
+            s_list[atomicAdd(&s_n, 1)] = make_int4(bx * CONTACT_BX, by * CONTACT_BY, z0, min(z0 + CONTACT_BZ / split, L.nz));
+        }
         __syncthreads();
         const int n = s_n;
         for (int k = 0; k < n; ++k) {
-            const int b = s_list[k] / split, part = s_list[k] % split;
-            const int x = (b % B.nbx) * CONTACT_BX + threadIdx.x, y = ((b / B.nbx) % B.nby) * CONTACT_BY + threadIdx.y;
-            const int z0 = (b / (B.nbx * B.nby)) * CONTACT_BZ + part * (CONTACT_BZ / split), z1 = z0 + CONTACT_BZ / split;
+            const int4 it = s_list[k];
+            const int x = it.x + threadIdx.x, y = it.y + threadIdx.y;
             if (x < L.nx && y < L.ny)
-                for (int z = z0; z < z1 && z < L.nz; ++z) contact_node<T, Q>(p, x, y, z);
+                for (int z = it.z; z < it.w; ++z) contact_node<T, Q>(p, x, y, z);
         }
         __syncthreads();
     }
