@@ -12,7 +12,9 @@ than L2, so no flush is needed between steps.  Prints ONE JSON line on stdout (r
 
 The same line carries `sizes` (256^3 and 512^3, fp32 and fp64: MLUPS and the HBM fraction at each, as the north star
 asks), `footprint` (bytes per node and total GB with and without populations, from lbwp_state_bytes of both
-schemes) and `cpu_baseline` (the oracle on the host cores: all cores and single thread, 128^3).
+schemes), `two_component` (the paper's own workload class: two-component fp32 at 128^3, 256^3 and
+512^3, with the near-contact force off and on) and `cpu_baseline` (the oracle on the host cores: all cores and single
+thread, 128^3).
 
 N > 1 (`--gpus N` under torchrun): ONE periodic box of n x n x (n N) nodes, decomposed into z slabs of n planes per
 rank (weak scaling), halo planes exchanged with the z neighbours after every step (NCCL send/recv; slabs.py);
@@ -57,6 +59,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sizes", action="store_true", help="skip the 256^3 / 512^3 fp32 / fp64 sub-record")
     ap.add_argument("--size-steps", type=int, default=50, help="timed steps per entry of the sizes sub-record")
+    ap.add_argument("--no-two-component", action="store_true",
+                    help="skip the two_component sub-record (128^3 / 256^3 / 512^3 fp32, with and without the near-contact force)")
     return ap.parse_args()
 
 
@@ -352,6 +356,31 @@ def main():
                           "mlups": r["algorithmic_bytes_per_node"] and r["achieved"] * 1e9 / r["algorithmic_bytes_per_node"] / 1e6,
                           "achieved_gbs": r["achieved"], "frac": r["frac"], "frac_of_8TBs_nominal": r["frac_of_8TBs_nominal"]})
 
+    # the paper's own workload class (two-component D3Q19 fp32 with near-contact forces at 128^3), and the
+    # same at the north star's sizes: the config-5 two-component recipe, with the force off and on (A_h = 0.02, h_c = 4)
+    two_component = None
+    if not a.no_two_component and not a.no_sizes and world == 1 and a.scheme == "moments" and a.ncomp == 1 and a.dtype == "f32":
+        two_component = []
+        for n, lattices in ((128, (19,)), (256, (19,)), (512, (19, 27))):
+            cfg = wl.sweep_case(n, 19, 2, "f32")          # the recipe does not depend on the lattice
+            m2 = wl.as_dtype(cfg["moments"], "f32")
+            for lat in lattices:
+                for A_h in (0.0, 0.02):
+                    b = copy.copy(a)
+                    b.n, b.lattice, b.ncomp, b.dtype = n, lat, 2, "f32"
+                    s2 = lbwp.Lbwp(m2, lattice=lat, dtype="f32", ncomp=2, tau=cfg["tau"], A=cfg["A"], beta=cfg["beta"],
+                                   kernel=a.kernel, device=local, A_h=A_h)
+                    nst = a.size_steps * (4 if n == 128 else 1)
+                    t = time_steps(torch, s2, nst, 5, barrier)
+                    r = roofline_record(b, s2.kernel_name, n ** 3, t, nst, s2.launches_per_step, peak, peak_src)
+                    two_component.append({"grid": n, "lattice": lat, "dtype": "f32", "near_contact_A_h": A_h, "kernel": r["kernel"],
+                                          "launches_per_step": r["launches_per_step"], "steps": nst, "step_ms": r["step_ms"],
+                                          "mlups": n ** 3 / (r["step_ms"] * 1e-3) / 1e6, "achieved_gbs": r["achieved"],
+                                          "frac": r["frac"], "algorithmic_bytes_per_node": r["algorithmic_bytes_per_node"]})
+                    s2.close()
+                    del s2
+            del m2, cfg
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -384,6 +413,7 @@ def main():
         "gpu_launches": a.steps * lps,
         "roofline": roofline_record(a, kname, nodes, ms, a.steps, lps, peak, peak_src),
         "sizes": sizes,
+        "two_component": two_component,
         "footprint": footprint,
         "paper_context": "622 MLUPS without / 277 MLUPS with populations: V100 16 GB, 128^3, two-component D3Q19, fp32, with near-contact forces (PAPER.md:158-163); another machine and workload, not the target",
     }

@@ -173,7 +173,8 @@ int lbwp_diagnostics_static(int device, int dtype, int ncomp, int nx, int ny, in
  * PAPER.md:163-167).  A rank's context is an ordinary periodic box whose first and last H planes are HALO planes:
  * copies of the neighbouring ranks' boundary planes (H = 1; H = 2 for ncomp == 2 moments, whose colour gradient
  * reaches two planes; H = floor(h_c) + 3 with the near-contact force, whose interface walk and the gradients on its
- * way reach floor(h_c) + 1 planes beyond the two the step leaves wrong).  One step of the decomposed box = lbwp_step(ctx, 1) on every rank, then every rank packs its
+ * way reach floor(h_c) + 1 planes beyond the two the step leaves wrong).
+ * One step of the decomposed box = lbwp_step(ctx, 1) on every rank, then every rank packs its
  * H lowest and H highest OWNED planes of the new state, sends them to its z neighbours (NCCL send/recv, or a peer
  * copy) and unpacks what it receives into its halo planes.  The planes the step computed INTO the halo are garbage
  * (the box wrapped onto itself there) and are overwritten by the unpack.  The packed format is the library's private
