@@ -132,8 +132,8 @@ __device__ __forceinline__ void contact_node(const ContactParams<T>& p, int x, i
 // keep the pass from paying 26 loads per node for that:
 //   k_contact_scan   reads rA once, coalesced, and stores min and max of rA over every box of CONTACT_BX x CONTACT_BY x
 //                    CONTACT_BZ nodes (range[0][box], range[1][box]; the last boxes may overhang the grid);
-//   k_contact_fixup  a persistent kernel (its CTAs share the boxes out round-robin): for every box it takes min and max over the box and its 26 neighbours (which
-//                    cover the box's halo of one node, periodic).  G_a = 6 (sum_{c_ia = +1} w_i rA_i - sum_{c_ia = -1}
+//   k_contact_fixup  a persistent kernel (its CTAs share the boxes out round-robin): for every box it takes min and max
+//                    over the box and its 26 neighbours (which cover the box's halo of one node, periodic).  G_a = 6 (sum_{c_ia = +1} w_i rA_i - sum_{c_ia = -1}
 //                    w_i rA_i) and sum_{c_ia = +1} w_i = 1/6 on both lattices, so |G_a| <= max - min and |G|^2 <=
 //                    3 (max - min)^2: where max - min < 0.02 every node of the box has |G|^2 <= 1.2e-3 < G_I^2 = 2.5e-3
 //                    and the box is skipped (exact: no node that gets a force is skipped).  The CTA runs steps 1-3 on
