@@ -375,8 +375,9 @@ struct Tma2gCtx final : lbwp_ctx {
         else k_contact_scan<T, 2><<<gs, blk, 0, stream>>>(cp.L, B, ra, (T*)grad);
         const int split = B.count() >= 64 * sms ? 1 : CONTACT_BZ;   // 128^3: 2048 boxes, 512^3: 131072
         // large grids: more CTAs than fit at once, so that the block scheduler evens out the SMs (measured: 32 per SM
-        // 2.89 ms per step at 512^3 against 2.92 with 8; at 128^3 8 per SM 0.106 ms against 0.114 with 32)
-        const int gf = (int)std::min<long long>((long long)B.count() * split, (split == 1 ? 32 : 8) * sms);
+        // 2.89 ms per step at 512^3 against 2.92 with 8); small grids: what is resident at once (128^3: 4 per SM
+        // 0.1047 ms per step, 8: 0.1056, 16: 0.1088, 32: 0.114)
+        const int gf = (int)std::min<long long>((long long)B.count() * split, (split == 1 ? 32 : 4) * sms);
         if (P.lattice == 27) k_contact_fixup<T, 27><<<gf, blk, 0, stream>>>(cp, B, (const T*)grad, split);
         else k_contact_fixup<T, 19><<<gf, blk, 0, stream>>>(cp, B, (const T*)grad, split);
         cudaError_t e = cudaGetLastError();
